@@ -1,0 +1,168 @@
+"""CPU oracle (TEST INFRASTRUCTURE, not the product).
+
+ctypes front end of oracle/mfc_oracle.c.  Only tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs may import this package.  It imports nothing from the CUDA
+package; it takes a plain description of the problem (any object with the attributes ndim, n, dx,
+fluids, bc_lo, bc_hi, weno_eps) and numpy arrays.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from pathlib import Path
+
+import numpy as np
+
+_HERE = Path(__file__).resolve().parent
+_SRC = _HERE / "mfc_oracle.c"
+_LIB = _HERE / "libmfc_oracle.so"
+NG = 3
+MAXF = 4
+
+
+class _Problem(C.Structure):
+    _fields_ = [
+        ("ndim", C.c_int),
+        ("nf", C.c_int),
+        ("n", C.c_int * 3),
+        ("dx", C.c_double * 3),
+        ("gamma", C.c_double * MAXF),
+        ("pi_inf", C.c_double * MAXF),
+        ("bc_lo", C.c_int * 3),
+        ("bc_hi", C.c_int * 3),
+        ("weno_eps", C.c_double),
+    ]
+
+
+def build(force: bool = False) -> Path:
+    """Compile the oracle with gcc (-O2, no FMA contraction, OpenMP on the outer loops only)."""
+    if force or not _LIB.exists() or _LIB.stat().st_mtime < _SRC.stat().st_mtime:
+        tmp = _LIB.with_suffix(f".so.tmp{os.getpid()}")
+        cmd = ["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC", "-std=c99",
+               str(_SRC), "-o", str(tmp), "-lm"]
+        subprocess.run(cmd, check=True)
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        L = C.CDLL(str(_LIB))
+        dp = C.POINTER(C.c_double)
+        pp = C.POINTER(_Problem)
+        L.orc_neq.argtypes = [pp]; L.orc_neq.restype = C.c_int
+        L.orc_elems.argtypes = [pp]; L.orc_elems.restype = C.c_longlong
+        L.orc_fill_ghosts.argtypes = [pp, dp]; L.orc_fill_ghosts.restype = None
+        L.orc_cons_to_prim.argtypes = [pp, dp, dp]; L.orc_cons_to_prim.restype = None
+        L.orc_cons_to_prim_cell.argtypes = [pp, dp, dp]; L.orc_cons_to_prim_cell.restype = None
+        L.orc_weno5.argtypes = [C.c_double] * 6 + [dp, dp]; L.orc_weno5.restype = None
+        L.orc_hllc.argtypes = [pp, C.c_int, dp, dp, dp, dp]; L.orc_hllc.restype = None
+        L.orc_line.argtypes = [pp, C.c_int, C.c_int, dp, dp, dp, dp, dp]; L.orc_line.restype = None
+        L.orc_rhs.argtypes = [pp, dp, dp]; L.orc_rhs.restype = None
+        L.orc_rk3_step.argtypes = [pp, dp, C.c_double]; L.orc_rk3_step.restype = None
+        L.orc_cfl_dt.argtypes = [pp, dp, C.c_double]; L.orc_cfl_dt.restype = C.c_double
+        L.orc_threads.argtypes = []; L.orc_threads.restype = C.c_int
+        L.orc_set_threads.argtypes = [C.c_int]; L.orc_set_threads.restype = None
+        _lib = L
+    return _lib
+
+
+def _dp(a: np.ndarray):
+    assert a.dtype == np.float64 and a.flags["C_CONTIGUOUS"]
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+class Oracle:
+    """The oracle bound to one problem description."""
+
+    def __init__(self, prob):
+        self.L = lib()
+        P = _Problem()
+        P.ndim = int(prob.ndim)
+        P.nf = len(prob.fluids)
+        assert 1 <= P.nf <= MAXF
+        for d in range(3):
+            P.n[d] = int(prob.n[d]) if d < prob.ndim else 1
+            P.dx[d] = float(prob.dx[d])
+            P.bc_lo[d] = int(prob.bc_lo[d])
+            P.bc_hi[d] = int(prob.bc_hi[d])
+        for i, (g, pinf) in enumerate(prob.fluids):
+            P.gamma[i] = float(g)
+            P.pi_inf[i] = float(pinf)
+        P.weno_eps = float(prob.weno_eps)
+        self.P = P
+        self.neq = self.L.orc_neq(C.byref(P))
+        self.elems = self.L.orc_elems(C.byref(P))
+        self.ndim = P.ndim
+        self.nf = P.nf
+
+    # -- whole-array operations (q is [neq, pz, py, px], modified in place where noted) --
+    def fill_ghosts(self, q: np.ndarray) -> None:
+        assert q.size == self.elems
+        self.L.orc_fill_ghosts(C.byref(self.P), _dp(q))
+
+    def cons_to_prim(self, q: np.ndarray) -> np.ndarray:
+        assert q.size == self.elems
+        w = np.empty_like(q)
+        self.L.orc_cons_to_prim(C.byref(self.P), _dp(q), _dp(w))
+        return w
+
+    def rhs(self, q: np.ndarray) -> np.ndarray:
+        """Returns L(q); fills q's ghost cells in place (as the C-ABI's mfc_rhs does)."""
+        assert q.size == self.elems
+        out = np.zeros_like(q)
+        self.L.orc_rhs(C.byref(self.P), _dp(q), _dp(out))
+        return out
+
+    def rk3_step(self, q: np.ndarray, dt: float) -> None:
+        assert q.size == self.elems
+        self.L.orc_rk3_step(C.byref(self.P), _dp(q), float(dt))
+
+    def cfl_dt(self, q: np.ndarray, cfl: float) -> float:
+        assert q.size == self.elems
+        return float(self.L.orc_cfl_dt(C.byref(self.P), _dp(q), float(cfl)))
+
+    # -- pieces, for pins --
+    def cons_to_prim_cell(self, qc) -> np.ndarray:
+        qc = np.ascontiguousarray(qc, dtype=np.float64)
+        w = np.empty(self.neq)
+        self.L.orc_cons_to_prim_cell(C.byref(self.P), _dp(qc), _dp(w))
+        return w
+
+    def hllc(self, direction: int, wL, wR):
+        wL = np.ascontiguousarray(wL, dtype=np.float64)
+        wR = np.ascontiguousarray(wR, dtype=np.float64)
+        F = np.empty(self.neq)
+        u = np.empty(1)
+        self.L.orc_hllc(C.byref(self.P), int(direction), _dp(wL), _dp(wR), _dp(F), _dp(u))
+        return F, float(u[0])
+
+    def line(self, direction: int, w: np.ndarray):
+        """w: [neq, n + 6] primitives on one line -> vL, vR [neq, n+2], F [neq, n+1], uf [n+1]."""
+        w = np.ascontiguousarray(w, dtype=np.float64)
+        n = w.shape[1] - 2 * NG
+        vL = np.empty((self.neq, n + 2)); vR = np.empty((self.neq, n + 2))
+        F = np.empty((self.neq, n + 1)); uf = np.empty(n + 1)
+        self.L.orc_line(C.byref(self.P), int(direction), n, _dp(w), _dp(vL), _dp(vR), _dp(F), _dp(uf))
+        return vL, vR, F, uf
+
+
+def weno5(a, b, c, d, e, eps=1e-16):
+    vL = C.c_double()
+    vR = C.c_double()
+    lib().orc_weno5(float(a), float(b), float(c), float(d), float(e), float(eps), C.byref(vL), C.byref(vR))
+    return vL.value, vR.value
+
+
+def threads() -> int:
+    return int(lib().orc_threads())
+
+
+def set_threads(n: int) -> None:
+    lib().orc_set_threads(int(n))

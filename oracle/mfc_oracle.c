@@ -1,0 +1,378 @@
+/*
+ * mfc_oracle.c  --  TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, fp64 CPU statement of what the hot path computes: the right-hand side of the
+ * 5-equation (Allaire, K = 0) diffuse-interface model with stiffened-gas EOS on a uniform grid,
+ * driven by 3-stage TVD Runge-Kutta, exactly in the paper's order:
+ *   ghost fill -> cons->prim -> per-direction WENO5-JS -> HLLC (+ face velocity) -> flux difference
+ *   + alpha*div(u) -> RK stage combine;  plus the CFL time step.
+ * Reference: /root/reference/PAPER.md (arxiv 2305.09163); every function cites the passage it follows.
+ * Where the paper is silent or garbled the reading is the one listed in DESIGN.md ("Readings", B1..B21).
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may build,
+ * load or call this file.  It shares no code, header, table or constant with the CUDA path
+ * (paper_2305_09163_b200/csrc/), and neither includes the other.
+ *
+ * No blocking, fusion or reordering beyond what the algorithm states: whole-array passes, one after the
+ * other.  The only parallelism is an OpenMP "parallel for" on the outermost loop of each pass (lines are
+ * independent), which changes no arithmetic.  Build: gcc -O2 -ffp-contract=off [-fopenmp] -shared -fPIC.
+ *
+ * Parity pins (tests/test_oracle_pins.py): every function below is pinned by something other than itself
+ * (closed forms, exact Riemann solutions, polynomial exactness, invariants, numpy.pad).  The Davis
+ * wave-speed estimate and the u_face formula are pinned only through consistency/invariants (C2, C5, C7,
+ * C8), not against MFC's own unpublished choice: "parity unpinned" w.r.t. MFC itself for those two readings.
+ *
+ * Layout: q[eq][k][j][i], i (x) fastest, padded by ng = 3 ghost cells on both sides of every active
+ * dimension (PAPER.md:238 flattened arrays; PAPER.md:168 buffers).  Equation order:
+ *   alpha_i rho_i (i = 1..nf), rho u_d (d = 1..ndim), rho E, alpha_i (i = 1..nf-1).      (reading B1)
+ */
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+
+#define ORC_NG 3
+#define ORC_MAXF 4
+#define ORC_MAXEQ (2 * ORC_MAXF + 3)
+
+typedef struct {
+    int ndim;              /* 1, 2, 3 */
+    int nf;                /* number of fluids */
+    int n[3];              /* interior cells (1 in inactive dimensions) */
+    double dx[3];          /* uniform spacing, Eq. (8) */
+    double gamma[ORC_MAXF];
+    double pi_inf[ORC_MAXF];
+    int bc_lo[3], bc_hi[3]; /* 0 periodic, 1 extrapolation */
+    double weno_eps;
+} orc_problem;
+
+static int neq_of(const orc_problem *P) { return 2 * P->nf + P->ndim; }
+static int pad_of(const orc_problem *P, int d) { return d < P->ndim ? P->n[d] + 2 * ORC_NG : 1; }
+static size_t cells_padded(const orc_problem *P) {
+    return (size_t)pad_of(P, 0) * (size_t)pad_of(P, 1) * (size_t)pad_of(P, 2);
+}
+/* i, j, k are padded indices */
+static size_t at(const orc_problem *P, int i, int j, int k) {
+    return ((size_t)k * (size_t)pad_of(P, 1) + (size_t)j) * (size_t)pad_of(P, 0) + (size_t)i;
+}
+
+int orc_neq(const orc_problem *P) { return neq_of(P); }
+long long orc_elems(const orc_problem *P) { return (long long)neq_of(P) * (long long)cells_padded(P); }
+
+/* ------------------------------------------------------------------------------------------------
+ * A3. Ghost fill.  PAPER.md:168 ("allocating buffers at the domain edges", size from the WENO order).
+ * Periodic: q[-m] = q[n-m], q[n-1+m] = q[m-1]; extrapolation: q[-m] = q[0], q[n-1+m] = q[n-1], m = 1..3.
+ * Dimensions in order x, y, z, each pass covering the full padded extent of the other dimensions.
+ * ---------------------------------------------------------------------------------------------- */
+void orc_fill_ghosts(const orc_problem *P, double *q)
+{
+    const int neq = neq_of(P);
+    const size_t C = cells_padded(P);
+    for (int d = 0; d < P->ndim; ++d) {
+        const int n = P->n[d];
+        int ext[3] = { pad_of(P, 0), pad_of(P, 1), pad_of(P, 2) };
+        ext[d] = 1;
+        for (int e = 0; e < neq; ++e) {
+            double *v = q + (size_t)e * C;
+            for (int c = 0; c < ext[2]; ++c)
+                for (int b = 0; b < ext[1]; ++b)
+                    for (int a = 0; a < ext[0]; ++a)
+                        for (int m = 1; m <= ORC_NG; ++m) {
+                            int idx[3] = { a, b, c };
+                            int src_lo = (P->bc_lo[d] == 0) ? (n - m) : 0;         /* interior index */
+                            int src_hi = (P->bc_hi[d] == 0) ? (m - 1) : (n - 1);
+                            size_t dst, src;
+                            idx[d] = ORC_NG - m;            dst = at(P, idx[0], idx[1], idx[2]);
+                            idx[d] = ORC_NG + src_lo;       src = at(P, idx[0], idx[1], idx[2]);
+                            v[dst] = v[src];
+                            idx[d] = ORC_NG + n - 1 + m;    dst = at(P, idx[0], idx[1], idx[2]);
+                            idx[d] = ORC_NG + src_hi;       src = at(P, idx[0], idx[1], idx[2]);
+                            v[dst] = v[src];
+                        }
+        }
+    }
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * A2. Mixture rules for the stiffened gas, PAPER.md:54-58 (Eq. 1): rho e = p/(gamma-1) + gamma pi/(gamma-1)
+ * per fluid; alpha-weighted for the mixture (reading B2): Gamma = sum alpha_i/(gamma_i-1),
+ * Pi = sum alpha_i gamma_i pi_i/(gamma_i-1), alpha_nf = 1 - sum_{i<nf} alpha_i.
+ * w is a primitive vector (alpha_i rho_i, u_d, p, alpha_i).
+ * ---------------------------------------------------------------------------------------------- */
+static void mixture(const orc_problem *P, const double *alpha_adv, double *Gam, double *Pi)
+{
+    const int nf = P->nf;
+    double last = 1.0, G = 0.0, Q = 0.0;
+    for (int i = 0; i < nf; ++i) {
+        double a;
+        if (i < nf - 1) { a = alpha_adv[i]; last -= a; } else { a = last; }
+        G += a / (P->gamma[i] - 1.0);
+        Q += a * P->gamma[i] * P->pi_inf[i] / (P->gamma[i] - 1.0);
+    }
+    *Gam = G; *Pi = Q;
+}
+
+/* A4. cons -> prim for one cell ("conservative variables q are converted to the primitive
+ * ones before reconstruction").  w = (alpha_i rho_i, u_d = rho u_d / rho, p, alpha_i),
+ * p = (rho E - rho|u|^2/2 - Pi)/Gamma. */
+void orc_cons_to_prim_cell(const orc_problem *P, const double *qc, double *w)
+{
+    const int nf = P->nf, D = P->ndim;
+    double rho = 0.0, ke = 0.0, Gam, Pi;
+    for (int i = 0; i < nf; ++i) { w[i] = qc[i]; rho += qc[i]; }
+    for (int d = 0; d < D; ++d) { w[nf + d] = qc[nf + d] / rho; ke += 0.5 * rho * w[nf + d] * w[nf + d]; }
+    for (int i = 0; i < nf - 1; ++i) w[nf + D + 1 + i] = qc[nf + D + 1 + i];
+    mixture(P, qc + nf + D + 1, &Gam, &Pi);
+    w[nf + D] = (qc[nf + D] - ke - Pi) / Gam;
+}
+
+/* whole padded array */
+void orc_cons_to_prim(const orc_problem *P, const double *q, double *w)
+{
+    const int neq = neq_of(P);
+    const size_t C = cells_padded(P);
+#pragma omp parallel for schedule(static)
+    for (long long c = 0; c < (long long)C; ++c) {
+        double qc[ORC_MAXEQ], wc[ORC_MAXEQ];
+        for (int e = 0; e < neq; ++e) qc[e] = q[(size_t)e * C + (size_t)c];
+        orc_cons_to_prim_cell(P, qc, wc);
+        for (int e = 0; e < neq; ++e) w[(size_t)e * C + (size_t)c] = wc[e];
+    }
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * A5. WENO5-JS, PAPER.md:143-150 (Eq. 12 with r = 0..k-1, k = 3; reading B6) and Listing 1
+ * (alpha = d/(beta**2), omega = alpha/sum(alpha), v = sum(omega*poly); eps added to
+ * beta, reading B8/B9).  Uniform-grid Jiang-Shu form.  Stencil a..e = w_{i-2..i+2}.
+ * vL = value at face i+1/2 seen from cell i; vR = value at face i-1/2 seen from cell i.
+ * ---------------------------------------------------------------------------------------------- */
+void orc_weno5(double a, double b, double c, double d, double e, double eps, double *vL, double *vR)
+{
+    const double b0 = 13.0 / 12.0 * (a - 2.0 * b + c) * (a - 2.0 * b + c) + 0.25 * (a - 4.0 * b + 3.0 * c) * (a - 4.0 * b + 3.0 * c);
+    const double b1 = 13.0 / 12.0 * (b - 2.0 * c + d) * (b - 2.0 * c + d) + 0.25 * (b - d) * (b - d);
+    const double b2 = 13.0 / 12.0 * (c - 2.0 * d + e) * (c - 2.0 * d + e) + 0.25 * (3.0 * c - 4.0 * d + e) * (3.0 * c - 4.0 * d + e);
+    const double d0 = 0.1, d1 = 0.6, d2 = 0.3;
+    {   /* left state at i+1/2 */
+        const double p0 = (2.0 * a - 7.0 * b + 11.0 * c) / 6.0;
+        const double p1 = (-b + 5.0 * c + 2.0 * d) / 6.0;
+        const double p2 = (2.0 * c + 5.0 * d - e) / 6.0;
+        const double a0 = d0 / ((b0 + eps) * (b0 + eps));
+        const double a1 = d1 / ((b1 + eps) * (b1 + eps));
+        const double a2 = d2 / ((b2 + eps) * (b2 + eps));
+        const double s = a0 + a1 + a2;
+        *vL = (a0 / s) * p0 + (a1 / s) * p1 + (a2 / s) * p2;
+    }
+    {   /* right state at i-1/2: mirror image (a<->e, b<->d), so beta_2, beta_1, beta_0 pair with d0, d1, d2 */
+        const double p0 = (2.0 * e - 7.0 * d + 11.0 * c) / 6.0;
+        const double p1 = (-d + 5.0 * c + 2.0 * b) / 6.0;
+        const double p2 = (2.0 * c + 5.0 * b - a) / 6.0;
+        const double a0 = d0 / ((b2 + eps) * (b2 + eps));
+        const double a1 = d1 / ((b1 + eps) * (b1 + eps));
+        const double a2 = d2 / ((b0 + eps) * (b0 + eps));
+        const double s = a0 + a1 + a2;
+        *vR = (a0 / s) * p0 + (a1 / s) * p1 + (a2 / s) * p2;
+    }
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * A6. HLLC, PAPER.md:152-164 (Eq. 13-14), with the face velocity of PAPER.md:126-136 (Eq. 10 and the
+ * garbled equation after section 3.2: the Riemann solver returns F and u; reading B5).
+ *   s_L = min(u_L - c_L, u_R - c_R), s_R = max(u_L + c_L, u_R + c_R)                  (reading B11)
+ *   s_* from continuity of normal velocity and pressure across the contact
+ *   Eq. 14: F = F(q_K) + s_K (q*_K - q_K) in the star regions, F(q_K) when supersonic; the missing fourth
+ *   case s_R <= 0 is F(q_R) (reading B7).  K = L if s_* >= 0 else R (reading B13).
+ *   alpha rows carry the quasi-conservative flux alpha*u; u_face is the HLLC flux of the constant 1
+ *   (reading B12), so F_alpha = alpha_K * u_face.
+ * dir: 0, 1, 2 = normal direction.  wL, wR: primitive vectors.  F: neq fluxes.
+ * ---------------------------------------------------------------------------------------------- */
+void orc_hllc(const orc_problem *P, int dir, const double *wL, const double *wR, double *F, double *uface)
+{
+    const int nf = P->nf, D = P->ndim, neq = neq_of(P);
+    const int iE = nf + D, iA = nf + D + 1;
+    double rho[2], E[2], c[2], un[2], p[2];
+    const double *w[2] = { wL, wR };
+    for (int K = 0; K < 2; ++K) {
+        double Gam, Pi, r = 0.0, ke = 0.0;
+        for (int i = 0; i < nf; ++i) r += w[K][i];
+        for (int d = 0; d < D; ++d) ke += 0.5 * r * w[K][nf + d] * w[K][nf + d];
+        mixture(P, w[K] + iA, &Gam, &Pi);
+        rho[K] = r;
+        p[K] = w[K][iE];
+        un[K] = w[K][nf + dir];
+        E[K] = Gam * p[K] + Pi + ke;                                  /* A2: rho E */
+        c[K] = sqrt(((Gam + 1.0) * p[K] + Pi) / (Gam * r));           /* A2: frozen mixture sound speed */
+    }
+    const double sL = fmin(un[0] - c[0], un[1] - c[1]);
+    const double sR = fmax(un[0] + c[0], un[1] + c[1]);
+    const double sS = (p[1] - p[0] + rho[0] * un[0] * (sL - un[0]) - rho[1] * un[1] * (sR - un[1]))
+                    / (rho[0] * (sL - un[0]) - rho[1] * (sR - un[1]));
+    const int K = (sS >= 0.0) ? 0 : 1;
+    const double sK = (K == 0) ? sL : sR;
+    const double shat = (K == 0) ? fmin(sL, 0.0) : fmax(sR, 0.0);
+    const double xi = (sK - un[K]) / (sK - sS);
+    const double *wk = w[K];
+    double qK[ORC_MAXEQ], qS[ORC_MAXEQ], FK[ORC_MAXEQ];
+    /* state q_K, physical flux F(q_K), star state q*_K */
+    for (int i = 0; i < nf; ++i) {
+        qK[i] = wk[i];
+        FK[i] = wk[i] * un[K];
+        qS[i] = xi * wk[i];
+    }
+    for (int d = 0; d < D; ++d) {
+        qK[nf + d] = rho[K] * wk[nf + d];
+        FK[nf + d] = rho[K] * wk[nf + d] * un[K] + ((d == dir) ? p[K] : 0.0);
+        qS[nf + d] = xi * rho[K] * ((d == dir) ? sS : wk[nf + d]);
+    }
+    qK[iE] = E[K];
+    FK[iE] = (E[K] + p[K]) * un[K];
+    qS[iE] = xi * (E[K] + (sS - un[K]) * (rho[K] * sS + p[K] / (sK - un[K])));
+    for (int i = 0; i < nf - 1; ++i) {
+        qK[iA + i] = wk[iA + i];
+        FK[iA + i] = wk[iA + i] * un[K];
+        qS[iA + i] = xi * wk[iA + i];
+    }
+    for (int e = 0; e < neq; ++e) F[e] = FK[e] + shat * (qS[e] - qK[e]);
+    *uface = un[K] + shat * (xi - 1.0);
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * A7. RHS, PAPER.md:105-130 (Eq. 6-10) with s(q) = 0 and h = -alpha on the alpha rows (K = 0):
+ *   L_k = sum_d (F^d_{k,-1/2} - F^d_{k,+1/2})/dx_d  [+ alpha_i * sum_d (u^d_{+1/2} - u^d_{-1/2})/dx_d]
+ * Fills the ghosts of q, converts to primitives, then direction by direction: WENO on every line,
+ * HLLC on every face, flux differences.  L has q's padded layout; only its interior is written.
+ * ---------------------------------------------------------------------------------------------- */
+void orc_rhs(const orc_problem *P, double *q, double *L)
+{
+    const int nf = P->nf, D = P->ndim, neq = neq_of(P);
+    const size_t C = cells_padded(P);
+    const int iA = nf + D + 1;
+    double *w = (double *)malloc(sizeof(double) * (size_t)neq * C);
+    orc_fill_ghosts(P, q);
+    orc_cons_to_prim(P, q, w);
+    memset(L, 0, sizeof(double) * (size_t)neq * C);
+
+    for (int dir = 0; dir < D; ++dir) {
+        const int n = P->n[dir];
+        /* the two other directions, interior only */
+        const int o1 = (dir + 1) % 3, o2 = (dir + 2) % 3;
+        const int n1 = P->n[o1], n2 = P->n[o2];
+        const int off1 = (o1 < D) ? ORC_NG : 0, off2 = (o2 < D) ? ORC_NG : 0;
+#pragma omp parallel for schedule(static)
+        for (int line = 0; line < n1 * n2; ++line) {
+            const int b = line % n1, cidx = line / n1;
+            /* per-line work arrays indexed by cell j = -1..n  ->  j+1 */
+            double *vL = (double *)malloc(sizeof(double) * (size_t)(n + 2) * neq);
+            double *vR = (double *)malloc(sizeof(double) * (size_t)(n + 2) * neq);
+            double *Ff = (double *)malloc(sizeof(double) * (size_t)(n + 1) * neq);
+            double *uf = (double *)malloc(sizeof(double) * (size_t)(n + 1));
+            int idx[3];
+            idx[o1] = off1 + b; idx[o2] = off2 + cidx;
+            /* WENO: cells j = -1..n */
+            for (int j = -1; j <= n; ++j) {
+                double st[5];
+                for (int e = 0; e < neq; ++e) {
+                    for (int s = -2; s <= 2; ++s) {
+                        idx[dir] = ORC_NG + j + s;
+                        st[s + 2] = w[(size_t)e * C + at(P, idx[0], idx[1], idx[2])];
+                    }
+                    orc_weno5(st[0], st[1], st[2], st[3], st[4], P->weno_eps,
+                              &vL[(size_t)(j + 1) * neq + e], &vR[(size_t)(j + 1) * neq + e]);
+                }
+            }
+            /* HLLC: faces f = j+1/2, j = -1..n-1; left state from cell j, right state from cell j+1
+             * */
+            for (int j = -1; j <= n - 1; ++j)
+                orc_hllc(P, dir, &vL[(size_t)(j + 1) * neq], &vR[(size_t)(j + 2) * neq],
+                         &Ff[(size_t)(j + 1) * neq], &uf[j + 1]);
+            /* flux difference, Eq. 9-10 */
+            for (int j = 0; j < n; ++j) {
+                size_t cell;
+                idx[dir] = ORC_NG + j;
+                cell = at(P, idx[0], idx[1], idx[2]);
+                for (int e = 0; e < neq; ++e)
+                    L[(size_t)e * C + cell] += (Ff[(size_t)j * neq + e] - Ff[(size_t)(j + 1) * neq + e]) / P->dx[dir];
+                for (int i = 0; i < nf - 1; ++i)
+                    L[(size_t)(iA + i) * C + cell] += q[(size_t)(iA + i) * C + cell] * (uf[j + 1] - uf[j]) / P->dx[dir];
+            }
+            free(vL); free(vR); free(Ff); free(uf);
+        }
+    }
+    free(w);
+}
+
+/* one direction's reconstructed states and fluxes on a single 1-D line of primitives, for unit pins and
+ * stage-by-stage parity: w[neq][n + 2 ng] -> vL, vR [neq][n+2] (cells -1..n), F [neq][n+1], uf [n+1] */
+void orc_line(const orc_problem *P, int dir, int n, const double *w, double *vL, double *vR, double *F, double *uf)
+{
+    const int neq = neq_of(P);
+    const int np = n + 2 * ORC_NG;
+    for (int j = -1; j <= n; ++j)
+        for (int e = 0; e < neq; ++e) {
+            const double *s = w + (size_t)e * np + ORC_NG + j;
+            orc_weno5(s[-2], s[-1], s[0], s[1], s[2], P->weno_eps, &vL[(size_t)e * (n + 2) + j + 1], &vR[(size_t)e * (n + 2) + j + 1]);
+        }
+    for (int j = -1; j <= n - 1; ++j) {
+        double wl[ORC_MAXEQ], wr[ORC_MAXEQ], f[ORC_MAXEQ];
+        for (int e = 0; e < neq; ++e) { wl[e] = vL[(size_t)e * (n + 2) + j + 1]; wr[e] = vR[(size_t)e * (n + 2) + j + 2]; }
+        orc_hllc(P, dir, wl, wr, f, &uf[j + 1]);
+        for (int e = 0; e < neq; ++e) F[(size_t)e * (n + 1) + j + 1] = f[e];
+    }
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * A8. 3-stage TVD (SSP) Runge-Kutta, PAPER.md:172 (ref. [19]; reading B16):
+ *   q1 = q + dt L(q);  q2 = 3/4 q + 1/4 (q1 + dt L(q1));  q <- 1/3 q + 2/3 (q2 + dt L(q2)).
+ * Interior cells only are updated; ghosts are refilled inside every L.
+ * ---------------------------------------------------------------------------------------------- */
+void orc_rk3_step(const orc_problem *P, double *q, double dt)
+{
+    const size_t N = (size_t)orc_elems(P);
+    double *q1 = (double *)malloc(sizeof(double) * N);
+    double *q2 = (double *)malloc(sizeof(double) * N);
+    double *L = (double *)malloc(sizeof(double) * N);
+    orc_rhs(P, q, L);
+#pragma omp parallel for schedule(static)
+    for (long long i = 0; i < (long long)N; ++i) q1[i] = q[i] + dt * L[i];
+    orc_rhs(P, q1, L);
+#pragma omp parallel for schedule(static)
+    for (long long i = 0; i < (long long)N; ++i) q2[i] = 0.75 * q[i] + 0.25 * (q1[i] + dt * L[i]);
+    orc_rhs(P, q2, L);
+#pragma omp parallel for schedule(static)
+    for (long long i = 0; i < (long long)N; ++i) q[i] = (1.0 / 3.0) * q[i] + (2.0 / 3.0) * (q2[i] + dt * L[i]);
+    free(q1); free(q2); free(L);
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * A9. CFL time step ("CFL-restricted time step"; reading B17):
+ *   dt = cfl * min over interior cells and directions of dx_d / (|u_d| + c).
+ * ---------------------------------------------------------------------------------------------- */
+double orc_cfl_dt(const orc_problem *P, const double *q, double cfl)
+{
+    const int nf = P->nf, D = P->ndim, neq = neq_of(P);
+    const size_t C = cells_padded(P);
+    double best = INFINITY;
+    for (int k = 0; k < P->n[2]; ++k)
+        for (int j = 0; j < P->n[1]; ++j)
+            for (int i = 0; i < P->n[0]; ++i) {
+                double qc[ORC_MAXEQ], w[ORC_MAXEQ], Gam, Pi, rho = 0.0, c;
+                size_t cell = at(P, i + ORC_NG, j + (D > 1 ? ORC_NG : 0), k + (D > 2 ? ORC_NG : 0));
+                for (int e = 0; e < neq; ++e) qc[e] = q[(size_t)e * C + cell];
+                orc_cons_to_prim_cell(P, qc, w);
+                for (int f = 0; f < nf; ++f) rho += w[f];
+                mixture(P, w + nf + D + 1, &Gam, &Pi);
+                c = sqrt(((Gam + 1.0) * w[nf + D] + Pi) / (Gam * rho));
+                for (int d = 0; d < D; ++d) {
+                    double t = P->dx[d] / (fabs(w[nf + d]) + c);
+                    if (t < best) best = t;
+                }
+            }
+    return cfl * best;
+}
+
+#ifdef _OPENMP
+#include <omp.h>
+int orc_threads(void) { return omp_get_max_threads(); }
+void orc_set_threads(int n) { omp_set_num_threads(n); }
+#else
+int orc_threads(void) { return 1; }
+void orc_set_threads(int n) { (void)n; }
+#endif
