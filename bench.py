@@ -1,0 +1,325 @@
+#!/usr/bin/env python
+"""Benchmark of the hot path (BASELINE.json metric): grind time, ns per (cell x equation x RHS evaluation), fp64.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg3] [--n 256]
+
+One "step" is one pass of the whole path over the workload: the CFL reduction (mfc_cfl_dt) and one 3-stage
+TVD-RK step (mfc_rk3_step = 3 x [cons->prim + ghost fill, WENO5+HLLC sweeps in x, y, z, flux difference, stage
+combine]).  The workload is BASELINE.json configs[3] (256^3 two-fluid bubble cloud), seeded and synthetic.
+N > 1 (torchrun): independent replicas, one per GPU, no data-path collective ("replicas only");
+time is the max over ranks and the value counts the cells of all ranks.
+
+--impl reference times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "grind_time_ns_per_cell_eqn_rhs"
+UNIT = "ns/(cell*eqn*RHS)"
+RHS_PER_STEP = 3
+FP64_NOMINAL_TFLOPS = 2 * 64 * 148 * 1.965e9 / 1e12   # 64 DFMA/clk/SM x 148 SMs x 1.965 GHz
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "measured"
+    return 6650.0, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons while the timed region runs (B200_PROFILING.md recipe)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.rows = []
+        self.proc = None
+        self.thread = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+            return
+        def pump():
+            for line in self.proc.stdout:
+                self.rows.append(line.strip())
+        self.thread = threading.Thread(target=pump, daemon=True)
+        self.thread.start()
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        if self.thread:
+            self.thread.join(timeout=2)
+        sm, smax, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); smax.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def get_workload(name: str, n: int | None):
+    from paper_2305_09163_b200 import workloads as wl
+    idx = int(name.replace("cfg", ""))
+    fn = wl.CONFIGS[idx]
+    return fn(n=n) if n else fn()
+
+
+# --------------------------------------------------------------------------------------------------------
+# algorithmic work of one sweep launch: per cell and direction
+# --------------------------------------------------------------------------------------------------------
+def sweep_algorithmic(prob, direction: int, rk_stage_mix: bool):
+    neq, nf, D = prob.neq, prob.nf, prob.ndim
+    flops = neq * 80 + (102 if nf <= 2 else 116) + 3 * neq      # WENO5 (common-denominator form) + HLLC + flux difference
+    last = direction == D - 1
+    rd = neq                                                    # primitives, once
+    wr = neq
+    if direction > 0:
+        rd += neq                                               # accumulated RHS
+    if last and rk_stage_mix:
+        rd += neq * (1 + 2 / 3)                                 # q_s every stage, q_n in stages 2 and 3
+    return flops, 8.0 * (rd + wr)
+
+
+def run_ours(args):
+    import torch
+
+    from paper_2305_09163_b200 import binding as B
+    from paper_2305_09163_b200 import build as mfc_build
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if rank == 0:
+        mfc_build.build()
+    if dist:
+        dist.barrier()
+    B.lib()
+
+    prob, q = get_workload(args.workload, args.n)
+    ctx = B.init_from_problem(prob, device=local, march_segment=args.segment)
+    neq, ng, padded, elems = B.mfc_layout(ctx)
+    stream = torch.cuda.current_stream().cuda_stream
+    q_host = torch.from_numpy(q).pin_memory()
+    qd = q_host.cuda(non_blocking=True)
+    torch.cuda.synchronize()
+
+    def step():
+        dt = B.mfc_cfl_dt(ctx, qd.data_ptr(), stream)
+        B.mfc_rk3_step(ctx, qd.data_ptr(), dt, stream)
+        return dt
+
+    for _ in range(max(3, args.warmup)):
+        step()
+    torch.cuda.synchronize()
+
+    def barrier():
+        if dist:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- timed region: exactly K steps, inputs resident in HBM ----
+    for kid in range(B.MFC_K_COUNT):
+        B.mfc_profile_get(ctx, kid, reset=True)
+    B.mfc_profile_enable(ctx, True)
+    sampler = ClockSampler(local) if rank == 0 else None
+    barrier()
+    if sampler:
+        sampler.start()
+    n0 = B.mfc_launch_count(ctx)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    barrier()
+    clocks = sampler.stop() if sampler else None
+    ms_total = e0.elapsed_time(e1)
+    launches = B.mfc_launch_count(ctx) - n0
+    prof = {}
+    for kid in range(B.MFC_K_COUNT):
+        n, ms = B.mfc_profile_get(ctx, kid, reset=True)
+        prof[B.KERNEL_NAMES[kid]] = {"launches": n, "ms_total": ms, "ms_avg": (ms / n if n else 0.0)}
+    B.mfc_profile_enable(ctx, False)
+    state_ok = bool(torch.isfinite(qd).all().item())
+
+    # ---- e2e: same step through the C ABI from HOST buffers (H2D + D2H inside the timed region) ----
+    q_host.copy_(torch.from_numpy(q))
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    B.mfc_advance_host(ctx, q_host.data_ptr(), 1, 0.0, stream)       # warm-up (allocates the library's device copy)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        B.mfc_advance_host(ctx, q_host.data_ptr(), 1, 0.0, stream)   # synchronous: returns after the D2H copy
+    torch.cuda.synchronize()
+    e2e_ms = (time.perf_counter() - t0) * 1e3 / e2e_steps
+
+    if dist:
+        t = torch.tensor([ms_total, e2e_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total, e2e_ms = float(t[0]), float(t[1])
+        ok = torch.tensor([1.0 if state_ok else 0.0], device="cuda")
+        dist.all_reduce(ok, op=dist.ReduceOp.MIN)
+        state_ok = bool(ok.item() > 0.5)
+
+    if rank == 0:
+        ms_step = ms_total / args.steps
+        work = prob.cells * world * neq * RHS_PER_STEP
+        grind = ms_step * 1e6 / work
+        hbm_peak, hbm_src = measured_peaks()
+        fp64_tf, fp64_ms = B.mfc_probe_dfma(local)
+        # dominant kernel = the sweep family with the largest share of the step
+        sweeps = [("sweep_x", 0), ("sweep_y", 1), ("sweep_z", 2)][:prob.ndim]
+        dom, ddir = max(sweeps, key=lambda s: prof[s[0]]["ms_total"])
+        flops_cell, bytes_cell = sweep_algorithmic(prob, ddir, True)
+        t_avg = prof[dom]["ms_avg"] * 1e-3
+        ach_gbs = bytes_cell * prob.cells / t_avg / 1e9
+        ach_tf = flops_cell * prob.cells / t_avg / 1e12
+        t_hbm = bytes_cell * prob.cells / (hbm_peak * 1e9)
+        t_alu = flops_cell * prob.cells / (fp64_tf * 1e12)
+        if t_hbm >= t_alu:
+            roof = {"kernel": dom, "bound": "hbm", "achieved": ach_gbs, "peak": hbm_peak, "unit": "GB/s",
+                    "frac": ach_gbs / hbm_peak, "traffic": None, "peak_source": f"MEASURED_PEAKS.json ({hbm_src})"}
+        else:
+            roof = {"kernel": dom, "bound": "alu", "achieved": ach_tf, "peak": fp64_tf, "unit": "TFLOP/s",
+                    "frac": ach_tf / fp64_tf, "traffic": None, "peak_source": "mfc_probe_dfma, measured in this run"}
+        roof.update({"algorithmic_flops_per_cell": flops_cell, "algorithmic_bytes_per_cell": bytes_cell,
+                     "avg_launch_ms": prof[dom]["ms_avg"], "hbm_frac": ach_gbs / hbm_peak, "fp64_frac": ach_tf / fp64_tf,
+                     "fp64_peak_measured_tflops": fp64_tf, "fp64_peak_nominal_tflops": FP64_NOMINAL_TFLOPS,
+                     "kernel_ms_sum_over_step_ms": sum(v["ms_total"] for v in prof.values()) / ms_total})
+        out = {
+            "metric": METRIC, "value": grind, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup),
+            "ms_per_step": ms_step, "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "impl": "ours",
+            "config": {"workload": f"{prob.name} {prob.n[0]}x{prob.n[1]}x{prob.n[2]} nf={prob.nf} neq={neq} (BASELINE.json configs[{args.workload[3:]}])",
+                       "cells_per_gpu": prob.cells, "rhs_per_step": RHS_PER_STEP, "parallelism": f"replicas x{world}",
+                       "l2": "inputs larger than L2 (each state array >= 1 GB at 256^3)", "march_segment": args.segment,
+                       "step": "mfc_cfl_dt + mfc_rk3_step"},
+            "cells_steps_per_s": prob.cells * world / (ms_step * 1e-3),
+            "gpu_launches": launches,
+            "kernels": prof,
+            "roofline": roof,
+            "e2e": {"value": e2e_ms * 1e6 / work, "unit": UNIT, "ms_per_step": e2e_ms, "steps": e2e_steps,
+                    "h2d_bytes_per_step": elems * 8, "d2h_bytes_per_step": elems * 8,
+                    "call": "mfc_advance_host(q_host pinned, nsteps=1, CFL dt)"},
+            "clocks": clocks, "state_finite": state_ok,
+        }
+        if world == 1 and not args.no_cpu:
+            out["cpu_baseline"] = cpu_baseline(args)
+        print(json.dumps(out))
+    B.mfc_destroy(ctx)
+    if dist:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+# --------------------------------------------------------------------------------------------------------
+# CPU oracle legs (the only places bench.py may execute oracle/)
+# --------------------------------------------------------------------------------------------------------
+def oracle_step_time(args, n_sample: int, steps: int, warmup: int):
+    import oracle
+    prob, q = get_workload(args.workload, n_sample)
+    orc = oracle.Oracle(prob)
+    times = []
+    for i in range(warmup + steps):
+        t0 = time.perf_counter()
+        dt = orc.cfl_dt(q, prob.cfl)
+        orc.rk3_step(q, dt)
+        if i >= warmup:
+            times.append(time.perf_counter() - t0)
+    return prob, times, oracle.threads()
+
+
+def cpu_baseline(args):
+    n_sample = args.cpu_n
+    prob, times, cores = oracle_step_time(args, n_sample, 2, 0)
+    sec = sum(times) / len(times)
+    return {"value": sec * 1e9 / (prob.cells * prob.neq * RHS_PER_STEP), "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{prob.name} shrunk to {n_sample}^3 cells, 2 steps of (CFL + RK3) with the OpenMP oracle, {sec:.2f} s/step"}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    n_sample = args.ref_n
+    prob, times, cores = oracle_step_time(args, n_sample, args.steps, min(args.warmup, 1))
+    sec = sum(times) / len(times)
+    grind = sec * 1e9 / (prob.cells * prob.neq * RHS_PER_STEP)
+    sample = f"{prob.name} shrunk to {n_sample}^3 cells per step (CPU oracle, OpenMP, {cores} threads)"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": grind, "unit": UNIT, "n_gpus": int(os.environ.get("WORLD_SIZE", "1")),
+        "steps": args.steps, "warmup": min(args.warmup, 1), "ms_per_step": sec * 1e3, "higher_is_better": False,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"{prob.name} (BASELINE.json configs[{args.workload[3:]}]), bounded sample {n_sample}^3", "rhs_per_step": RHS_PER_STEP},
+        "cpu_baseline": {"value": grind, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": grind, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg3", choices=["cfg0", "cfg1", "cfg2", "cfg3", "cfg4"])
+    ap.add_argument("--n", type=int, default=None, help="override cells per dimension (default: the config's size)")
+    ap.add_argument("--segment", type=int, default=0, help="marching segment of the y/z sweeps (0 = heuristic)")
+    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--cpu-n", type=int, default=128, help="cells per dimension of the cpu_baseline sample")
+    ap.add_argument("--ref-n", type=int, default=96, help="cells per dimension of the --impl reference sample")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

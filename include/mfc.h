@@ -1,0 +1,150 @@
+/*
+ * mfc.h -- C ABI of libmfc_b200: the right-hand side of the 5-equation diffuse-interface model
+ * (Allaire form, K = 0) with stiffened-gas EOS on a uniform structured grid, as hand-written CUDA for
+ * sm_100a (NVIDIA B200), driven by 3-stage TVD Runge-Kutta.
+ *
+ * Method: arxiv 2305.09163 (Radhakrishnan et al.), cited below as PAPER.md:LINE (section / equation).
+ * Readings of passages where the paper is silent or garbled are listed in DESIGN.md ("Readings", B1..B21).
+ *
+ * Conventions shared by every entry point
+ * ---------------------------------------
+ * State layout ("flattened multidimensional arrays", Listing 1 index order (j,k,l,i)):
+ *   q[eq][z][y][x], x fastest, fp64, padded by ng = 3 cells on both sides of every ACTIVE dimension
+ *   (buffers sized by the WENO order); an inactive dimension has extent 1.
+ *   Equation order (NEQ = 2*n_fluids + ndim, reading B1):
+ *     alpha_i rho_i (i = 1..n_fluids), rho u_d (d = 1..ndim), rho E, alpha_i (i = 1..n_fluids-1).
+ *   mfc_layout() returns the padded extents and the element count of one such array.
+ * Pointers: names ending in _dev are DEVICE pointers (e.g. a torch tensor's data_ptr()) on the device
+ *   given to mfc_init; names ending in _host are HOST pointers.  The caller owns every buffer it passes;
+ *   the library owns its scratch (primitive array, stage buffer, RHS accumulator, reduction workspace),
+ *   allocated in mfc_init and released in mfc_destroy.
+ * Boundary conditions are applied while the primitive array is built (ghost cells of the primitive array
+ *   are computed from the wrapped / clamped interior cell).  Ghost cells of q are therefore
+ *   never read and never written; ghost entries of rhs are unspecified.
+ * Streams: `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  All work is
+ *   enqueued on it.  Only mfc_cfl_dt, mfc_advance_host, mfc_profile_get and mfc_probe_dfma synchronise.
+ * Errors: every function returns MFC_OK (0) or a negative mfc_status; nothing is thrown or printed.
+ *   A context is not thread-safe.  State admissibility is not checked on the hot path: non-finite or
+ *   inadmissible states propagate as NaN.  There is no CPU fallback: without a CUDA device mfc_init fails
+ *   with MFC_ECUDA.
+ */
+#ifndef MFC_B200_H
+#define MFC_B200_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MFC_NG 3         /* ghost layers (WENO5) */
+#define MFC_MAX_FLUIDS 3 /* compiled template set: ndim in {1,2,3} x n_fluids in {1,2,3} */
+
+typedef enum {
+    MFC_OK = 0,
+    MFC_EINVAL = -1,       /* null pointer, bad shape, n_d < 3 in an active dimension, gamma <= 1, bad BC kind */
+    MFC_EUNSUPPORTED = -2, /* (ndim, n_fluids) outside the compiled template set */
+    MFC_ECUDA = -3,        /* CUDA runtime error (sticky); no device */
+    MFC_ENOMEM = -4        /* device or host allocation failed */
+} mfc_status;
+
+/* uniform grid, PAPER.md:105-124 (Eq. 6-9): dx_d = (hi_d - lo_d) / n_d */
+typedef struct {
+    int ndim;        /* 1, 2 or 3 */
+    int n[3];        /* interior cells; entries >= ndim are ignored (treated as 1) */
+    double lo[3], hi[3];
+} mfc_grid;
+
+/* stiffened gas, PAPER.md:54-58 (Eq. 1) */
+typedef struct {
+    double gamma, pi_inf;
+} mfc_fluid;
+
+typedef enum { MFC_BC_PERIODIC = 0, MFC_BC_EXTRAP = 1 } mfc_bc_kind;
+
+/* ghost-cell fills; periodic must be set on both sides of a dimension or on neither */
+typedef struct {
+    int lo[3], hi[3]; /* mfc_bc_kind per side of each dimension */
+} mfc_bc;
+
+typedef struct {
+    double weno_eps;   /* WENO-JS epsilon, Eq. 12 / Listing 1; <= 0 selects 1e-16 */
+    double cfl;        /* CFL number used by mfc_cfl_dt; <= 0 selects 0.3 */
+    int device;        /* CUDA device ordinal; < 0 selects the current device */
+    int march_segment; /* cells each thread marches in the y / z sweeps; <= 0 selects a heuristic */
+} mfc_opts;
+
+typedef struct mfc_ctx mfc_ctx;
+
+/* Creates a context: validates (ndim, n_fluids) against the compiled template set, stores the EOS and BC
+ * tables, allocates scratch (3 state-sized arrays).  eos: n_fluids entries.  opts may be NULL. */
+int mfc_init(mfc_ctx **out, const mfc_grid *grid, int n_fluids, const mfc_fluid *eos, const mfc_bc *bc,
+             const mfc_opts *opts);
+
+void mfc_destroy(mfc_ctx *ctx);
+
+/* Layout query: neq, ng, padded extents (x, y, z) and elements of one state array (neq * prod padded).
+ * Any out pointer may be NULL. */
+int mfc_layout(const mfc_ctx *ctx, int *neq, int *ng, long long padded_n[3], long long *elems);
+
+/* L(q): one evaluation of the spatial operator, PAPER.md:105-130 (Eq. 6-10) with s(q) = 0, K = 0:
+ *   cons->prim with ghost fill -> per direction WENO5-JS (Eq. 12,
+ *   Listing 1) -> HLLC flux and face velocity (Eq. 13-14) ->
+ *   rhs_k = sum_d (F_{k,-1/2} - F_{k,+1/2})/dx_d  [+ alpha_i sum_d (u_{+1/2} - u_{-1/2})/dx_d on alpha rows].
+ * q_dev is read (interior only); the interior of rhs_dev is written.  q_dev and rhs_dev must not alias. */
+int mfc_rhs(mfc_ctx *ctx, const double *q_dev, double *rhs_dev, void *stream);
+
+/* One 3-stage TVD Runge-Kutta step of size dt, in place on the interior of q_dev (ref. [19]):
+ *   q1 = q + dt L(q);  q2 = 3/4 q + 1/4 (q1 + dt L(q1));  q <- 1/3 q + 2/3 (q2 + dt L(q2)). */
+int mfc_rk3_step(mfc_ctx *ctx, double *q_dev, double dt, void *stream);
+
+/* CFL-restricted time step: dt = cfl * min over interior cells and directions of
+ * dx_d / (|u_d| + c), c the frozen mixture sound speed.  Synchronises `stream`; writes one host double. */
+int mfc_cfl_dt(mfc_ctx *ctx, const double *q_dev, double *dt_host, void *stream);
+
+/* Whole path from HOST memory: copies q_host to the device, takes nsteps RK3 steps (each with
+ * dt = dt_fixed if dt_fixed > 0, else the CFL step of the current state), copies the state back into
+ * q_host and synchronises.  t_host (may be NULL) receives the sum of the steps taken.
+ * q_host: `elems` doubles in the layout above; pinned memory makes the copies asynchronous. */
+int mfc_advance_host(mfc_ctx *ctx, double *q_host, int nsteps, double dt_fixed, double *t_host, void *stream);
+
+/* ---- stage outputs, for parity tests of the individual steps of the path ---- */
+
+/* a0 + a1: primitive array w = (alpha_i rho_i, u_d, p, alpha_i) on the whole padded box, ghost cells taken
+ * from the wrapped / clamped interior cell of q_dev.  w_dev: `elems` doubles. */
+int mfc_cons_to_prim(mfc_ctx *ctx, const double *q_dev, double *w_dev, void *stream);
+
+/* a2 + a3 on one line of primitives with normal direction dir (0,1,2 < ndim), using the same device
+ * functions as the sweeps.  w_dev: [neq][n + 6]; vL_dev, vR_dev: [neq][n + 2] (cells -1..n: state at face
+ * i+1/2 resp. i-1/2 seen from cell i); F_dev: [neq][n + 1]; uface_dev: [n + 1] (faces -1/2 .. n-1/2). */
+int mfc_line_fluxes(mfc_ctx *ctx, int dir, int n, const double *w_dev, double *vL_dev, double *vR_dev,
+                    double *F_dev, double *uface_dev, void *stream);
+
+/* ---- measurement hooks ---- */
+
+typedef enum {
+    MFC_K_PRIM = 0,    /* cons->prim + ghost fill */
+    MFC_K_SWEEP_X = 1, /* fused WENO5 + HLLC + flux difference, x */
+    MFC_K_SWEEP_Y = 2,
+    MFC_K_SWEEP_Z = 3,
+    MFC_K_CFL = 4,
+    MFC_K_COUNT = 5
+} mfc_kernel_id;
+
+/* With profiling on, every kernel launch is bracketed by CUDA events on its own stream. */
+int mfc_profile_enable(mfc_ctx *ctx, int on);
+/* Synchronises outstanding event pairs, then returns launches and summed device milliseconds of one kernel
+ * family since the last reset.  reset != 0 clears the accumulators of that family afterwards. */
+int mfc_profile_get(mfc_ctx *ctx, int kernel_id, long long *launches, double *total_ms, int reset);
+/* Number of kernels this context has launched since mfc_init (all families). */
+long long mfc_launch_count(const mfc_ctx *ctx);
+
+/* FP64 FMA micro-benchmark (register-resident dependent DFMA chains on every SM) used as the measured
+ * ALU roofline denominator.  Returns TFLOP/s (2 flops per DFMA) and the launch time in ms. */
+int mfc_probe_dfma(int device, double *tflops_host, double *ms_host);
+
+const char *mfc_strerror(int code);
+const char *mfc_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MFC_B200_H */

@@ -1,0 +1,513 @@
+// C ABI of libmfc_b200 (include/mfc.h): context, scratch memory, the order of launches of one RHS evaluation
+// and of the 3-stage TVD Runge-Kutta step, the CFL reduction, the host-buffer entry point and the
+// measurement hooks.  No arithmetic of the method lives here: every step of the path runs in the kernels
+// of mfc_device.cuh.  No CPU fallback.
+#include "../../include/mfc.h"
+#include "mfc_launch.h"
+
+#include <cmath>
+#include <cstring>
+#include <new>
+#include <vector>
+
+namespace mfc {
+
+cudaError_t launch_prim(int ndim, int nf, const Geo &g, const Eos &e, const double *q, double *w, cudaStream_t s)
+{
+    switch (ndim) {
+        case 1: return launch_prim_d1(nf, g, e, q, w, s);
+        case 2: return launch_prim_d2(nf, g, e, q, w, s);
+        case 3: return launch_prim_d3(nf, g, e, q, w, s);
+    }
+    return cudaErrorInvalidValue;
+}
+cudaError_t launch_sweep(int ndim, int nf, int dir, const Geo &g, const Eos &e, const double *w, const SweepOut &o,
+                         int segment, cudaStream_t s)
+{
+    switch (ndim) {
+        case 1: return launch_sweep_d1(nf, dir, g, e, w, o, segment, s);
+        case 2: return launch_sweep_d2(nf, dir, g, e, w, o, segment, s);
+        case 3: return launch_sweep_d3(nf, dir, g, e, w, o, segment, s);
+    }
+    return cudaErrorInvalidValue;
+}
+cudaError_t launch_cfl(int ndim, int nf, const Geo &g, const Eos &e, const double *q, unsigned long long *min_bits,
+                       cudaStream_t s)
+{
+    switch (ndim) {
+        case 1: return launch_cfl_d1(nf, g, e, q, min_bits, s);
+        case 2: return launch_cfl_d2(nf, g, e, q, min_bits, s);
+        case 3: return launch_cfl_d3(nf, g, e, q, min_bits, s);
+    }
+    return cudaErrorInvalidValue;
+}
+cudaError_t launch_line(int ndim, int nf, int dir, const Eos &e, int n, const double *w, double *vL, double *vR,
+                        double *F, double *uf, cudaStream_t s)
+{
+    switch (ndim) {
+        case 1: return launch_line_d1(nf, dir, e, n, w, vL, vR, F, uf, s);
+        case 2: return launch_line_d2(nf, dir, e, n, w, vL, vR, F, uf, s);
+        case 3: return launch_line_d3(nf, dir, e, n, w, vL, vR, F, uf, s);
+    }
+    return cudaErrorInvalidValue;
+}
+
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceGuard(int dev)
+    {
+        if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = cudaSetDevice(dev) == cudaSuccess;
+    }
+    ~DeviceGuard()
+    {
+        if (switched) cudaSetDevice(prev);
+    }
+};
+
+struct EventPair {
+    cudaEvent_t a, b;
+    int kid;
+};
+
+}  // namespace mfc
+
+struct mfc_ctx {
+    int ndim = 0, nf = 0, neq = 0, device = 0, segment = 0;
+    double cfl = 0.3;
+    long long elems = 0;
+    mfc::Geo g{};
+    mfc::Eos e{};
+    double *w = nullptr, *q1 = nullptr, *acc = nullptr, *q_own = nullptr;
+    unsigned long long *min_dev = nullptr;
+    unsigned long long *min_host = nullptr;  // pinned
+    bool profile = false;
+    std::vector<mfc::EventPair> pending;
+    std::vector<cudaEvent_t> pool;
+    double ms[MFC_K_COUNT] = {0, 0, 0, 0, 0};
+    long long launches[MFC_K_COUNT] = {0, 0, 0, 0, 0};
+    long long launch_total = 0;
+};
+
+namespace {
+
+using namespace mfc;
+
+int flush_events(mfc_ctx *c)
+{
+    for (auto &p : c->pending) {
+        if (cudaEventSynchronize(p.b) != cudaSuccess) return MFC_ECUDA;
+        float t = 0.f;
+        if (cudaEventElapsedTime(&t, p.a, p.b) != cudaSuccess) return MFC_ECUDA;
+        c->ms[p.kid] += (double)t;
+        c->pool.push_back(p.a);
+        c->pool.push_back(p.b);
+    }
+    c->pending.clear();
+    return MFC_OK;
+}
+
+cudaEvent_t get_event(mfc_ctx *c)
+{
+    if (!c->pool.empty()) {
+        cudaEvent_t e = c->pool.back();
+        c->pool.pop_back();
+        return e;
+    }
+    cudaEvent_t e = nullptr;
+    cudaEventCreate(&e);
+    return e;
+}
+
+// brackets one kernel launch with events when profiling is on, and counts it
+struct Timed {
+    mfc_ctx *c;
+    int kid;
+    cudaStream_t s;
+    cudaEvent_t a = nullptr, b = nullptr;
+    Timed(mfc_ctx *c_, int kid_, cudaStream_t s_) : c(c_), kid(kid_), s(s_)
+    {
+        if (c->profile) {
+            if (c->pending.size() >= 8192) flush_events(c);
+            a = get_event(c);
+            b = get_event(c);
+            cudaEventRecord(a, s);
+        }
+    }
+    ~Timed()
+    {
+        c->launches[kid] += 1;
+        c->launch_total += 1;
+        if (a) {
+            cudaEventRecord(b, s);
+            c->pending.push_back({a, b, kid});
+        }
+    }
+};
+
+int cuda_to_status(cudaError_t e)
+{
+    if (e == cudaSuccess) return MFC_OK;
+    if (e == cudaErrorMemoryAllocation) return MFC_ENOMEM;
+    return MFC_ECUDA;
+}
+
+// One evaluation of L on the primitive array built from q_in; `fin` describes what the last sweep emits.
+int eval_L(mfc_ctx *c, const double *q_in, double *acc, SweepOut fin, cudaStream_t s)
+{
+    cudaError_t err;
+    {
+        Timed t(c, MFC_K_PRIM, s);
+        err = launch_prim(c->ndim, c->nf, c->g, c->e, q_in, c->w, s);
+    }
+    if (err != cudaSuccess) return cuda_to_status(err);
+    for (int dir = 0; dir < c->ndim; ++dir) {
+        SweepOut o = fin;
+        if (dir != c->ndim - 1) {
+            o.rk = 0;
+            o.acc_out = acc;
+        }
+        o.acc_in = dir == 0 ? nullptr : acc;
+        {
+            Timed t(c, MFC_K_SWEEP_X + dir, s);
+            err = launch_sweep(c->ndim, c->nf, dir, c->g, c->e, c->w, o, c->segment, s);
+        }
+        if (err != cudaSuccess) return cuda_to_status(err);
+    }
+    return MFC_OK;
+}
+
+int rk3(mfc_ctx *c, double *q, double dt, cudaStream_t s)
+{
+    SweepOut f{};
+    f.rk = 1;
+    f.dt = dt;
+    // q1 = q + dt L(q)
+    f.qn = q; f.qs = q; f.out = c->q1; f.ca = 0.0; f.cb = 1.0;
+    int st = eval_L(c, q, c->acc, f, s);
+    if (st) return st;
+    // q2 = 3/4 q + 1/4 (q1 + dt L(q1)), in place over q1 (the sweeps read the primitive array, not q1)
+    f.qn = q; f.qs = c->q1; f.out = c->q1; f.ca = 0.75; f.cb = 0.25;
+    st = eval_L(c, c->q1, c->acc, f, s);
+    if (st) return st;
+    // q <- 1/3 q + 2/3 (q2 + dt L(q2))
+    f.qn = q; f.qs = c->q1; f.out = q; f.ca = 1.0 / 3.0; f.cb = 2.0 / 3.0;
+    return eval_L(c, c->q1, c->acc, f, s);
+}
+
+int cfl_dt(mfc_ctx *c, const double *q, double *dt_host, cudaStream_t s)
+{
+    if (cudaMemsetAsync(c->min_dev, 0x7f, sizeof(unsigned long long), s) != cudaSuccess) return MFC_ECUDA;
+    cudaError_t err;
+    {
+        Timed t(c, MFC_K_CFL, s);
+        err = launch_cfl(c->ndim, c->nf, c->g, c->e, q, c->min_dev, s);
+    }
+    if (err != cudaSuccess) return cuda_to_status(err);
+    if (cudaMemcpyAsync(c->min_host, c->min_dev, sizeof(unsigned long long), cudaMemcpyDeviceToHost, s) != cudaSuccess)
+        return MFC_ECUDA;
+    if (cudaStreamSynchronize(s) != cudaSuccess) return MFC_ECUDA;
+    double v;
+    std::memcpy(&v, c->min_host, sizeof(double));
+    *dt_host = c->cfl * v;
+    return MFC_OK;
+}
+
+__global__ void __launch_bounds__(256) dfma_probe_kernel(double *out, int iters, double m, double a)
+{
+    double x0 = threadIdx.x * 1e-3, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            x0 = fma(x0, m, a); x1 = fma(x1, m, a); x2 = fma(x2, m, a); x3 = fma(x3, m, a);
+            x4 = fma(x4, m, a); x5 = fma(x5, m, a); x6 = fma(x6, m, a); x7 = fma(x7, m, a);
+        }
+    }
+    out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *mfc_strerror(int code)
+{
+    switch (code) {
+        case MFC_OK: return "ok";
+        case MFC_EINVAL: return "invalid argument";
+        case MFC_EUNSUPPORTED: return "(ndim, n_fluids) not in the compiled template set";
+        case MFC_ECUDA: return "CUDA runtime error";
+        case MFC_ENOMEM: return "out of memory";
+    }
+    return "unknown error";
+}
+
+const char *mfc_version(void) { return "mfc-b200 0.1 (sm_100a)"; }
+
+int mfc_init(mfc_ctx **out, const mfc_grid *grid, int n_fluids, const mfc_fluid *eos, const mfc_bc *bc, const mfc_opts *opts)
+{
+    if (!out || !grid || !eos || !bc) return MFC_EINVAL;
+    *out = nullptr;
+    if (grid->ndim < 1 || grid->ndim > 3 || n_fluids < 1) return MFC_EINVAL;
+    if (n_fluids > MFC_MAX_FLUIDS) return MFC_EUNSUPPORTED;
+    for (int d = 0; d < grid->ndim; ++d) {
+        if (grid->n[d] < MFC_NG || !(grid->hi[d] > grid->lo[d])) return MFC_EINVAL;
+        if (bc->lo[d] != MFC_BC_PERIODIC && bc->lo[d] != MFC_BC_EXTRAP) return MFC_EINVAL;
+        if (bc->hi[d] != MFC_BC_PERIODIC && bc->hi[d] != MFC_BC_EXTRAP) return MFC_EINVAL;
+        if ((bc->lo[d] == MFC_BC_PERIODIC) != (bc->hi[d] == MFC_BC_PERIODIC)) return MFC_EINVAL;
+    }
+    for (int i = 0; i < n_fluids; ++i)
+        if (!(eos[i].gamma > 1.0) || !std::isfinite(eos[i].gamma) || !std::isfinite(eos[i].pi_inf)) return MFC_EINVAL;
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return MFC_ECUDA;
+    int dev = opts ? opts->device : -1;
+    if (dev < 0 && cudaGetDevice(&dev) != cudaSuccess) return MFC_ECUDA;
+    if (dev >= ndev) return MFC_EINVAL;
+
+    mfc_ctx *c = new (std::nothrow) mfc_ctx();
+    if (!c) return MFC_ENOMEM;
+    c->ndim = grid->ndim;
+    c->nf = n_fluids;
+    c->neq = 2 * n_fluids + grid->ndim;
+    c->device = dev;
+    c->cfl = (opts && opts->cfl > 0.0) ? opts->cfl : 0.3;
+    const double eps = (opts && opts->weno_eps > 0.0) ? opts->weno_eps : 1.0e-16;
+
+    Geo &g = c->g;
+    g.ndim = grid->ndim;
+    for (int d = 0; d < 3; ++d) {
+        const bool act = d < grid->ndim;
+        g.n[d] = act ? grid->n[d] : 1;
+        g.g[d] = act ? NG : 0;
+        g.p[d] = g.n[d] + 2 * g.g[d];
+        g.inv_dx[d] = act ? (double)grid->n[d] / (grid->hi[d] - grid->lo[d]) : 1.0;
+        g.bc_lo[d] = act ? bc->lo[d] : MFC_BC_EXTRAP;
+        g.bc_hi[d] = act ? bc->hi[d] : MFC_BC_EXTRAP;
+    }
+    g.sy = g.p[0];
+    g.sz = (long long)g.p[0] * g.p[1];
+    g.cells = g.sz * g.p[2];
+    c->elems = g.cells * c->neq;
+
+    Eos &e = c->e;
+    std::memset(&e, 0, sizeof(e));
+    double Gm[MAX_NF], Pm[MAX_NF];
+    for (int i = 0; i < n_fluids; ++i) {
+        e.gamma[i] = eos[i].gamma;
+        e.pi_inf[i] = eos[i].pi_inf;
+        e.gm1[i] = eos[i].gamma - 1.0;
+        Gm[i] = 1.0 / (eos[i].gamma - 1.0);
+        Pm[i] = eos[i].gamma * eos[i].pi_inf / (eos[i].gamma - 1.0);
+    }
+    e.G_last = Gm[n_fluids - 1];
+    e.P_last = Pm[n_fluids - 1];
+    for (int i = 0; i < n_fluids - 1; ++i) {
+        e.dG[i] = Gm[i] - e.G_last;
+        e.dP[i] = Pm[i] - e.P_last;
+    }
+    e.weno_eps4 = 4.0 * eps;
+
+    // marching segment: enough threads for ~6 waves of 148 SMs x 256 resident threads, at least 32 cells
+    if (opts && opts->march_segment > 0) {
+        c->segment = opts->march_segment;
+    } else {
+        int seg = 1 << 30;
+        for (int dir = 1; dir < g.ndim; ++dir) {
+            const long long lines = (long long)g.n[0] * g.n[dir == 1 ? 2 : 1];
+            const long long want = (6LL * 148 * 256 + lines - 1) / lines;
+            int s = (int)((g.n[dir] + want - 1) / want);
+            if (s < 32) s = 32;
+            if (s < seg) seg = s;
+        }
+        c->segment = seg;
+    }
+
+    DeviceGuard guard(dev);
+    const size_t bytes = (size_t)c->elems * sizeof(double);
+    cudaError_t err = cudaMalloc((void **)&c->w, bytes);
+    if (err == cudaSuccess) err = cudaMalloc((void **)&c->q1, bytes);
+    if (err == cudaSuccess) err = cudaMalloc((void **)&c->acc, bytes);
+    if (err == cudaSuccess) err = cudaMalloc((void **)&c->min_dev, sizeof(unsigned long long));
+    if (err == cudaSuccess) err = cudaMallocHost((void **)&c->min_host, sizeof(unsigned long long));
+    if (err != cudaSuccess) {
+        const int st = cuda_to_status(err);
+        cudaGetLastError();
+        mfc_destroy(c);
+        return st;
+    }
+    *out = c;
+    return MFC_OK;
+}
+
+void mfc_destroy(mfc_ctx *c)
+{
+    if (!c) return;
+    {
+        DeviceGuard guard(c->device);
+        flush_events(c);
+        for (cudaEvent_t ev : c->pool) cudaEventDestroy(ev);
+        cudaFree(c->w);
+        cudaFree(c->q1);
+        cudaFree(c->acc);
+        cudaFree(c->q_own);
+        cudaFree(c->min_dev);
+        if (c->min_host) cudaFreeHost(c->min_host);
+    }
+    delete c;
+}
+
+int mfc_layout(const mfc_ctx *c, int *neq, int *ng, long long padded_n[3], long long *elems)
+{
+    if (!c) return MFC_EINVAL;
+    if (neq) *neq = c->neq;
+    if (ng) *ng = MFC_NG;
+    if (padded_n)
+        for (int d = 0; d < 3; ++d) padded_n[d] = c->g.p[d];
+    if (elems) *elems = c->elems;
+    return MFC_OK;
+}
+
+int mfc_rhs(mfc_ctx *c, const double *q_dev, double *rhs_dev, void *stream)
+{
+    if (!c || !q_dev || !rhs_dev || q_dev == rhs_dev) return MFC_EINVAL;
+    DeviceGuard guard(c->device);
+    SweepOut f{};
+    f.rk = 0;
+    f.acc_out = rhs_dev;
+    return eval_L(c, q_dev, rhs_dev, f, (cudaStream_t)stream);
+}
+
+int mfc_rk3_step(mfc_ctx *c, double *q_dev, double dt, void *stream)
+{
+    if (!c || !q_dev) return MFC_EINVAL;
+    DeviceGuard guard(c->device);
+    return rk3(c, q_dev, dt, (cudaStream_t)stream);
+}
+
+int mfc_cfl_dt(mfc_ctx *c, const double *q_dev, double *dt_host, void *stream)
+{
+    if (!c || !q_dev || !dt_host) return MFC_EINVAL;
+    DeviceGuard guard(c->device);
+    return cfl_dt(c, q_dev, dt_host, (cudaStream_t)stream);
+}
+
+int mfc_advance_host(mfc_ctx *c, double *q_host, int nsteps, double dt_fixed, double *t_host, void *stream)
+{
+    if (!c || !q_host || nsteps < 0) return MFC_EINVAL;
+    DeviceGuard guard(c->device);
+    cudaStream_t s = (cudaStream_t)stream;
+    const size_t bytes = (size_t)c->elems * sizeof(double);
+    if (!c->q_own) {
+        cudaError_t err = cudaMalloc((void **)&c->q_own, bytes);
+        if (err != cudaSuccess) {
+            cudaGetLastError();
+            return cuda_to_status(err);
+        }
+    }
+    if (cudaMemcpyAsync(c->q_own, q_host, bytes, cudaMemcpyHostToDevice, s) != cudaSuccess) return MFC_ECUDA;
+    double t = 0.0;
+    for (int it = 0; it < nsteps; ++it) {
+        double dt = dt_fixed;
+        if (!(dt_fixed > 0.0)) {
+            const int st = cfl_dt(c, c->q_own, &dt, s);
+            if (st) return st;
+        }
+        const int st = rk3(c, c->q_own, dt, s);
+        if (st) return st;
+        t += dt;
+    }
+    if (cudaMemcpyAsync(q_host, c->q_own, bytes, cudaMemcpyDeviceToHost, s) != cudaSuccess) return MFC_ECUDA;
+    if (cudaStreamSynchronize(s) != cudaSuccess) return MFC_ECUDA;
+    if (t_host) *t_host = t;
+    return MFC_OK;
+}
+
+int mfc_cons_to_prim(mfc_ctx *c, const double *q_dev, double *w_dev, void *stream)
+{
+    if (!c || !q_dev || !w_dev || q_dev == w_dev) return MFC_EINVAL;
+    DeviceGuard guard(c->device);
+    cudaError_t err;
+    {
+        Timed t(c, MFC_K_PRIM, (cudaStream_t)stream);
+        err = launch_prim(c->ndim, c->nf, c->g, c->e, q_dev, w_dev, (cudaStream_t)stream);
+    }
+    return cuda_to_status(err);
+}
+
+int mfc_line_fluxes(mfc_ctx *c, int dir, int n, const double *w_dev, double *vL_dev, double *vR_dev, double *F_dev,
+                    double *uface_dev, void *stream)
+{
+    if (!c || !w_dev || !vL_dev || !vR_dev || !F_dev || !uface_dev || n < 1 || dir < 0 || dir >= c->ndim) return MFC_EINVAL;
+    DeviceGuard guard(c->device);
+    c->launch_total += 2;
+    return cuda_to_status(launch_line(c->ndim, c->nf, dir, c->e, n, w_dev, vL_dev, vR_dev, F_dev, uface_dev, (cudaStream_t)stream));
+}
+
+int mfc_profile_enable(mfc_ctx *c, int on)
+{
+    if (!c) return MFC_EINVAL;
+    DeviceGuard guard(c->device);
+    if (!on) {
+        const int st = flush_events(c);
+        if (st) return st;
+    }
+    c->profile = on != 0;
+    return MFC_OK;
+}
+
+int mfc_profile_get(mfc_ctx *c, int kernel_id, long long *launches, double *total_ms, int reset)
+{
+    if (!c || kernel_id < 0 || kernel_id >= MFC_K_COUNT) return MFC_EINVAL;
+    DeviceGuard guard(c->device);
+    const int st = flush_events(c);
+    if (st) return st;
+    if (launches) *launches = c->launches[kernel_id];
+    if (total_ms) *total_ms = c->ms[kernel_id];
+    if (reset) {
+        c->launches[kernel_id] = 0;
+        c->ms[kernel_id] = 0.0;
+    }
+    return MFC_OK;
+}
+
+long long mfc_launch_count(const mfc_ctx *c) { return c ? c->launch_total : 0; }
+
+int mfc_probe_dfma(int device, double *tflops_host, double *ms_host)
+{
+    if (!tflops_host) return MFC_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return MFC_ECUDA;
+    if (device < 0 && cudaGetDevice(&device) != cudaSuccess) return MFC_ECUDA;
+    if (device >= ndev) return MFC_EINVAL;
+    DeviceGuard guard(device);
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) return MFC_ECUDA;
+    const int blocks = prop.multiProcessorCount * 8, threads = 256, iters = 8192;
+    double *out = nullptr;
+    if (cudaMalloc((void **)&out, sizeof(double) * (size_t)blocks * threads) != cudaSuccess) return MFC_ENOMEM;
+    cudaEvent_t a, b;
+    cudaEventCreate(&a);
+    cudaEventCreate(&b);
+    float best = 1e30f;
+    for (int rep = 0; rep < 4; ++rep) {
+        cudaEventRecord(a, 0);
+        dfma_probe_kernel<<<blocks, threads>>>(out, iters, 1.0 - 1e-9, 1e-9);
+        cudaEventRecord(b, 0);
+        cudaEventSynchronize(b);
+        float t = 0.f;
+        cudaEventElapsedTime(&t, a, b);
+        if (rep > 0 && t < best) best = t;
+    }
+    const cudaError_t err = cudaGetLastError();
+    cudaEventDestroy(a);
+    cudaEventDestroy(b);
+    cudaFree(out);
+    if (err != cudaSuccess) return MFC_ECUDA;
+    const double flops = 2.0 * 32.0 * (double)iters * (double)blocks * (double)threads;
+    *tflops_host = flops / ((double)best * 1e-3) / 1e12;
+    if (ms_host) *ms_host = (double)best;
+    return MFC_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,69 @@
+// Host-side description of one launch of each kernel family.  Plain structs passed by value to the kernels;
+// the per-dimension translation units (mfc_inst_d{1,2,3}.cu) implement the launchers declared at the end.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace mfc {
+
+constexpr int NG = 3;        // ghost layers, PAPER.md:168 (WENO5 stencil)
+constexpr int MAX_NF = 3;
+
+// padded box, x fastest (Listing 1 index order)
+struct Geo {
+    int ndim;
+    int n[3];            // interior cells (1 in inactive dimensions)
+    int p[3];            // padded extents (n + 2 NG in active dimensions, else 1)
+    int g[3];            // ghost offset per dimension (NG if active, else 0)
+    long long sy, sz;    // strides of y and z in cells (sx = 1)
+    long long cells;     // p[0] * p[1] * p[2] : stride between equations
+    double inv_dx[3];
+    int bc_lo[3], bc_hi[3];
+};
+
+// stiffened-gas tables, PAPER.md:54-58 (Eq. 1), alpha-weighted mixture (reading B2)
+struct Eos {
+    // as given / as the definition divides by: used by the cons->prim kernel, which evaluates the
+    // definition term by term without contraction
+    double gamma[MAX_NF], pi_inf[MAX_NF], gm1[MAX_NF];
+    // Gamma = G_last + sum_{i<nf-1} alpha_i dG_i ;  Pi likewise  (alpha_nf = 1 - sum alpha_i)
+    double G_last, P_last, dG[MAX_NF], dP[MAX_NF];
+    double weno_eps4;    // 4 * eps : smoothness indicators are carried scaled by 4
+};
+
+// output stage of a sweep: total = (acc_in ? acc_in[cell] : 0) + this direction's contribution;
+//   rk == 0 : acc_out[cell] = total
+//   rk == 1 : out[cell] = ca * qn[cell] + cb * (qs[cell] + dt * total)
+struct SweepOut {
+    const double *acc_in;
+    double *acc_out;
+    const double *qn, *qs;
+    double *out;
+    double ca, cb, dt;
+    int rk;
+};
+
+struct KernelTimer;  // opaque to the launchers
+
+cudaError_t launch_prim(int ndim, int nf, const Geo &g, const Eos &e, const double *q, double *w, cudaStream_t s);
+cudaError_t launch_sweep(int ndim, int nf, int dir, const Geo &g, const Eos &e, const double *w, const SweepOut &o,
+                         int segment, cudaStream_t s);
+cudaError_t launch_cfl(int ndim, int nf, const Geo &g, const Eos &e, const double *q, unsigned long long *min_bits,
+                       cudaStream_t s);
+cudaError_t launch_line(int ndim, int nf, int dir, const Eos &e, int n, const double *w, double *vL, double *vR,
+                        double *F, double *uf, cudaStream_t s);
+
+// per-dimension implementations
+#define MFC_DECL_DIM(D)                                                                                               \
+    cudaError_t launch_prim_d##D(int nf, const Geo &g, const Eos &e, const double *q, double *w, cudaStream_t s);     \
+    cudaError_t launch_sweep_d##D(int nf, int dir, const Geo &g, const Eos &e, const double *w, const SweepOut &o,    \
+                                  int segment, cudaStream_t s);                                                       \
+    cudaError_t launch_cfl_d##D(int nf, const Geo &g, const Eos &e, const double *q, unsigned long long *min_bits,    \
+                                cudaStream_t s);                                                                      \
+    cudaError_t launch_line_d##D(int nf, int dir, const Eos &e, int n, const double *w, double *vL, double *vR,       \
+                                 double *F, double *uf, cudaStream_t s);
+MFC_DECL_DIM(1)
+MFC_DECL_DIM(2)
+MFC_DECL_DIM(3)
+#undef MFC_DECL_DIM
+
+}  // namespace mfc

@@ -173,6 +173,19 @@ def rankine_hugoniot_stiffened(rho1: float, p1: float, gamma: float, pi_inf: flo
     return float(rho2), float(u2), float(p2)
 
 
+def diffuse_interface(dist: np.ndarray, h: float, cells: float) -> np.ndarray:
+    """Volume fraction of the fluid on the negative side of a signed distance `dist`: a tanh profile
+    `cells` grid cells wide, floored to [1e-6, 1-1e-6].  A diffuse-interface method needs the interface
+    resolved over a few cells; a one-cell staircase of alpha = 1e-6 | 1-1e-6 on a sphere makes WENO5
+    overshoot alpha below 0 at the single-cell caps and the unlimited scheme of the paper (no positivity
+    fix is mentioned) then produces NaN in the ORACLE itself within a few steps."""
+    a = 0.5 * (1.0 - np.tanh(dist / (cells * h)))
+    return np.clip(a, 1.0e-6, 1.0 - 1.0e-6)
+
+
+INTERFACE_CELLS = 1.5
+
+
 def cfg2(n: int = 128) -> Tuple[Problem, np.ndarray]:
     nn, lo, hi = _grid(3, (n, n, n))
     prob = Problem("cfg2_shock_bubble_3d", 3, nn, lo, hi, [WATER, AIR], (BC_EXTRAP,) * 3, (BC_EXTRAP,) * 3,
@@ -180,8 +193,9 @@ def cfg2(n: int = 128) -> Tuple[Problem, np.ndarray]:
     x = prob.centers(0)[None, None, :]
     y = prob.centers(1)[None, :, None]
     z = prob.centers(2)[:, None, None]
-    inside = (x - 0.5) ** 2 + (y - 0.5) ** 2 + (z - 0.5) ** 2 < 0.15 ** 2
-    a_air = np.where(inside, 1.0 - 1.0e-6, 1.0e-6)
+    dist = np.sqrt((x - 0.5) ** 2 + (y - 0.5) ** 2 + (z - 0.5) ** 2) - 0.15
+    a_air = diffuse_interface(dist, prob.dx[0], INTERFACE_CELLS)
+    inside = dist < 0.0
     rho2, u2, p2 = rankine_hugoniot_stiffened(1000.0, 1.0e5, WATER[0], WATER[1], 1.5)
     post = np.broadcast_to(x < 0.1, inside.shape)
     rho_w = np.where(post, rho2, 1000.0)
@@ -202,18 +216,22 @@ def cfg3(n: int = 256, seed: int = 2002, nbubbles: int = 64) -> Tuple[Problem, n
     centers = rng.uniform(0.2, 0.8, size=(nbubbles, 3))
     radii = np.exp(rng.normal(np.log(0.03), 0.3, size=nbubbles))
     xc, yc, zc = prob.centers(0), prob.centers(1), prob.centers(2)
-    inside = np.zeros((n, n, n), dtype=bool)
+    # signed distance to the union of the spheres (min over bubbles), evaluated in a box around each bubble
+    h = prob.dx[0]
+    pad = 8.0 * INTERFACE_CELLS * h            # tanh(8) = 1 - 2e-7: beyond this the floor 1e-6 applies anyway
+    dist = np.full((n, n, n), pad)
     for (cx, cy, cz), r in zip(centers, radii):
-        ix = np.nonzero(np.abs(xc - cx) < r)[0]
-        iy = np.nonzero(np.abs(yc - cy) < r)[0]
-        iz = np.nonzero(np.abs(zc - cz) < r)[0]
+        ix = np.nonzero(np.abs(xc - cx) < r + pad)[0]
+        iy = np.nonzero(np.abs(yc - cy) < r + pad)[0]
+        iz = np.nonzero(np.abs(zc - cz) < r + pad)[0]
         if len(ix) == 0 or len(iy) == 0 or len(iz) == 0:
             continue
         sx, sy, sz = (slice(ix[0], ix[-1] + 1), slice(iy[0], iy[-1] + 1), slice(iz[0], iz[-1] + 1))
-        d2 = ((xc[sx][None, None, :] - cx) ** 2 + (yc[sy][None, :, None] - cy) ** 2
-              + (zc[sz][:, None, None] - cz) ** 2)
-        inside[sz, sy, sx] |= d2 < r * r
-    a_air = np.where(inside, 1.0 - 1.0e-6, 1.0e-6)
+        d = np.sqrt((xc[sx][None, None, :] - cx) ** 2 + (yc[sy][None, :, None] - cy) ** 2
+                    + (zc[sz][:, None, None] - cz) ** 2) - r
+        dist[sz, sy, sx] = np.minimum(dist[sz, sy, sx], d)
+    a_air = diffuse_interface(dist, h, INTERFACE_CELLS)
+    inside = dist < 0.0
     p = np.where(np.broadcast_to(xc[None, None, :] < 0.05, inside.shape), 1.0e7, 1.0e5)
     q = assemble(prob, [1.0 - a_air, a_air], [1000.0, 1.2], [0.0, 0.0, 0.0], p)
     return prob, q

@@ -1,0 +1,406 @@
+"""GPU-vs-oracle parity through the C ABI (needs a B200: `-m gpu`).
+
+Bars (BASELINE.json north_star): max relative error per conserved variable <= 1e-10 after one RHS evaluation
+and <= 1e-8 after 10 RK3 steps, fp64, in the norm of DESIGN.md "Parity norm".  The cons->prim stage is held to
+bit equality.  Inputs are the seeded generators of workloads.py.
+"""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+
+import oracle
+from gpu_util import Gpu, parity_errors
+from paper_2305_09163_b200 import binding as B
+from paper_2305_09163_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+RHS_TOL = 1.0e-10
+RK_TOL = 1.0e-8
+TEMPLATE_SET = [(1, 1), (1, 2), (1, 3), (2, 1), (2, 2), (2, 3), (3, 1), (3, 2), (3, 3)]
+# several tiles of every kernel plus ragged tails: x blocks of 254 cells, marching segments of 8
+SIZES = {1: (1201,), 2: (301, 45), 3: (67, 29, 41)}
+
+
+def alpha_floor(prob, orc, q):
+    """1e-6 * max alpha * max (|u|+c)/dx, from the oracle's CFL step: max (|u|+c)/dx = cfl/dt."""
+    return 1.0e-6 / orc.cfl_dt(q, 1.0)
+
+
+def check_rhs(prob, q, tol=RHS_TOL, **kw):
+    orc = oracle.Oracle(prob)
+    qo = q.copy()
+    ref = orc.rhs(qo)
+    with Gpu(prob, **kw) as g:
+        got = g.rhs(q)
+    err = parity_errors(prob, got, ref, alpha_floor(prob, orc, qo))
+    assert np.all(err <= tol), f"{prob.name}: per-equation RHS error {err}"
+    return err
+
+
+# ---------------------------------------------------------------------------------------------
+# a0 + a1: ghost fill and cons->prim, bit for bit
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("ndim,nf", TEMPLATE_SET)
+@pytest.mark.parametrize("periodic", [True, False])
+def test_prim_array_is_bit_identical(ndim, nf, periodic):
+    n = {1: (37,), 2: (19, 11), 3: (9, 7, 5)}[ndim]
+    prob, q = wl.random_state(ndim, n, nf, seed=3, periodic=periodic)
+    orc = oracle.Oracle(prob)
+    qo = q.copy()
+    orc.fill_ghosts(qo)
+    ref = orc.cons_to_prim(qo)
+    with Gpu(prob) as g:
+        got = g.prim(q)
+    assert np.array_equal(got, ref)
+
+
+def test_prim_mixed_boundary_kinds():
+    prob, q = wl.random_state(3, (8, 6, 5), 2, seed=6, periodic=True)
+    prob.bc_lo = (wl.BC_EXTRAP, wl.BC_PERIODIC, wl.BC_EXTRAP)
+    prob.bc_hi = (wl.BC_EXTRAP, wl.BC_PERIODIC, wl.BC_EXTRAP)
+    orc = oracle.Oracle(prob)
+    qo = q.copy()
+    orc.fill_ghosts(qo)
+    ref = orc.cons_to_prim(qo)
+    with Gpu(prob) as g:
+        got = g.prim(q)
+    assert np.array_equal(got, ref)
+
+
+def test_ghost_cells_of_q_are_not_touched():
+    prob, q = wl.random_state(2, (12, 9), 2, seed=8, periodic=True)
+    q[...] = np.where(q == 0.0, 12345.0, q)  # mark the ghosts
+    with Gpu(prob) as g:
+        qd = g.to_dev(q)
+        out = g.torch.zeros_like(qd)
+        B.mfc_rhs(g.ctx, qd.data_ptr(), out.data_ptr(), g.stream)
+        B.mfc_rk3_step(g.ctx, qd.data_ptr(), 1e-9, g.stream)
+        g.torch.cuda.synchronize()
+        after = qd.cpu().numpy()
+    mask = np.ones(q.shape, dtype=bool)
+    mask[prob.interior()] = False
+    assert np.array_equal(after[mask], q[mask])
+
+
+# ---------------------------------------------------------------------------------------------
+# a2 + a3: WENO5 face states and HLLC fluxes on one line
+# ---------------------------------------------------------------------------------------------
+def random_prim_line(prob, n, rng, smooth):
+    nf, D = prob.nf, prob.ndim
+    x = np.linspace(0, 1, n + 2 * wl.NG)
+    rough = (lambda a: a * rng.uniform(-1, 1, size=x.size) + 0.5 * (rng.uniform(size=x.size) < 0.05)) if not smooth else (lambda a: 0.0)
+    z = [np.sin(2 * np.pi * (i + 1) * x + rng.uniform(0, 6)) + rough(0.3) for i in range(nf)]
+    e = [np.exp(1.5 * zi) for zi in z]
+    alpha = [np.clip(ei / sum(e), 1e-6, 1.0) for ei in e]
+    if nf > 1:
+        alpha[-1] = 1.0 - sum(alpha[:-1])
+    else:
+        alpha = [np.ones_like(x)]
+    rho0 = [1000.0, 1.2, 0.6][:nf]
+    w = np.zeros((prob.neq, x.size))
+    for i in range(nf):
+        w[i] = alpha[i] * rho0[i] * (1 + 0.1 * np.sin(5 * x + i) + rough(0.05))
+        if i < nf - 1:
+            w[nf + D + 1 + i] = alpha[i]
+    for d in range(D):
+        w[nf + d] = 400.0 * (np.sin(3 * x + d) + rough(0.5))      # sub- and supersonic in air-rich cells
+    w[nf + D] = 1.0e5 * np.exp(np.sin(4 * x) + rough(0.5))
+    return w
+
+
+@pytest.mark.parametrize("ndim,nf", TEMPLATE_SET)
+@pytest.mark.parametrize("smooth", [True, False])
+def test_line_face_states_and_fluxes(ndim, nf, smooth):
+    n = 777
+    prob, _ = wl.random_state(ndim, {1: (8,), 2: (8, 8), 3: (8, 8, 8)}[ndim], nf, seed=1)
+    orc = oracle.Oracle(prob)
+    rng = np.random.default_rng(100 * ndim + nf)
+    with Gpu(prob) as g:
+        for direction in range(ndim):
+            w = random_prim_line(prob, n, rng, smooth)
+            rL, rR, rF, ru = orc.line(direction, w)
+            gL, gR, gF, gu = g.line(direction, w)
+            for e in range(prob.neq):
+                s = np.max(np.abs(w[e])) + 1e-300
+                # reconstructed values: a few ulp of the local data
+                assert np.max(np.abs(gL[e] - rL[e])) <= 1e-13 * s, (direction, e)
+                assert np.max(np.abs(gR[e] - rR[e])) <= 1e-13 * s, (direction, e)
+            # fluxes: HLLC applied to each side's own face states (rounding differences of the states are
+            # amplified by the wave-speed switches only up to continuity)
+            for e in range(prob.neq):
+                s = np.max(np.abs(rF[e])) + 1e-300
+                assert np.max(np.abs(gF[e] - rF[e])) <= 1e-11 * s, (direction, e)
+            assert np.max(np.abs(gu - ru)) <= 1e-11 * np.max(np.abs(ru))
+
+
+@pytest.mark.parametrize("ndim,nf", [(1, 2), (3, 2), (3, 3)])
+def test_hllc_kernel_on_identical_inputs(ndim, nf):
+    """HLLC alone: feed the GPU Riemann solver the oracle's own face states by making them exact:
+    a piecewise-constant line has vL = vR = cell value wherever the stencil is constant."""
+    prob, _ = wl.random_state(ndim, {1: (8,), 3: (8, 8, 8)}[ndim], nf, seed=1)
+    orc = oracle.Oracle(prob)
+    rng = np.random.default_rng(7)
+    n = 600
+    base = random_prim_line(prob, n // 6 + 1, rng, smooth=False)[:, : n // 6 + 1]
+    w = np.repeat(base, 6, axis=1)[:, : n + 2 * wl.NG]          # plateaus of 6 cells
+    with Gpu(prob) as g:
+        for direction in range(ndim):
+            rL, rR, rF, ru = orc.line(direction, w)
+            gL, gR, gF, gu = g.line(direction, w)
+            for e in range(prob.neq):
+                s = np.max(np.abs(rF[e])) + 1e-300
+                assert np.max(np.abs(gF[e] - rF[e])) <= 1e-12 * s, (direction, e)
+
+
+# ---------------------------------------------------------------------------------------------
+# a0..a4: one RHS evaluation, every template instantiation, ragged sizes, small marching segments
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("ndim,nf", TEMPLATE_SET)
+@pytest.mark.parametrize("periodic", [True, False])
+def test_rhs_parity_random_states(ndim, nf, periodic):
+    prob, q = wl.random_state(ndim, SIZES[ndim], nf, seed=10 * ndim + nf, periodic=periodic)
+    check_rhs(prob, q, march_segment=8)
+
+
+@pytest.mark.parametrize("seg", [1, 5, 32, 1000])
+def test_rhs_is_independent_of_the_marching_segment(seg):
+    prob, q = wl.random_state(3, (40, 33, 37), 2, seed=77, periodic=False)
+    with Gpu(prob, march_segment=7) as g:
+        ref = g.rhs(q)
+    with Gpu(prob, march_segment=seg) as g:
+        got = g.rhs(q)
+    it = prob.interior()
+    assert np.array_equal(got[it], ref[it])
+
+
+@pytest.mark.parametrize("ndim,n", [(1, (3,)), (2, (3, 3)), (3, (3, 3, 3)), (3, (3, 300, 4)), (2, (255, 3)), (1, (254,)), (1, (255,))])
+def test_rhs_parity_smallest_and_tile_edge_sizes(ndim, n):
+    prob, q = wl.random_state(ndim, n, 2, seed=5, periodic=True, rough=False)
+    check_rhs(prob, q)
+
+
+@pytest.mark.parametrize("ndim,nf,periodic", [(1, 2, False), (2, 2, True), (3, 2, False), (3, 3, True)])
+def test_uniform_state_has_exactly_zero_rhs_on_gpu(ndim, nf, periodic):
+    prob, q = wl.random_state(ndim, SIZES[ndim], nf, seed=2, periodic=periodic)
+    it = prob.interior()
+    q[it] = q[it][:, :1, :1, :1]                 # one admissible cell everywhere
+    with Gpu(prob, march_segment=8) as g:
+        got = g.rhs(q)
+    assert np.all(got[it] == 0.0)
+
+
+def test_rhs_parity_cfg0():
+    prob, q = wl.cfg0()
+    check_rhs(prob, q)
+
+
+def test_rhs_parity_cfg1():
+    prob, q = wl.cfg1()
+    check_rhs(prob, q)
+
+
+def test_rhs_parity_cfg2():
+    prob, q = wl.cfg2()
+    check_rhs(prob, q)
+
+
+def test_rhs_parity_cfg4_reduced():
+    prob, q = wl.cfg4(n=96)
+    check_rhs(prob, q)
+
+
+# ---------------------------------------------------------------------------------------------
+# full sizes in the launch configuration bench.py times: sampled sub-boxes the oracle can compute
+# (L at a cell depends on the 6 axis neighbours up to distance 3 only) plus size-independent properties
+# ---------------------------------------------------------------------------------------------
+def subbox_reference(prob, q_full, lo, b):
+    """oracle L on the b^3 cells starting at interior index lo, from a (b+6)^3 cut-out of q_full."""
+    D = prob.ndim
+    idx = [np.arange(lo[d] - wl.NG, lo[d] + b + wl.NG) % prob.n[d] + wl.NG for d in range(D)]   # wrap: periodic cut-outs
+    cut = q_full[np.ix_(np.arange(prob.neq), idx[2], idx[1], idx[0])]
+    sub = wl.Problem("sub", D, (b + 6,) * 3, (0.0,) * 3, tuple((b + 6) * prob.dx[d] for d in range(3)), prob.fluids,
+                     (wl.BC_EXTRAP,) * 3, (wl.BC_EXTRAP,) * 3, weno_eps=prob.weno_eps)
+    qs = np.zeros(sub.shape())
+    qs[sub.interior()] = cut
+    L = oracle.Oracle(sub).rhs(qs)
+    return L[sub.interior()][:, wl.NG:-wl.NG, wl.NG:-wl.NG, wl.NG:-wl.NG]
+
+
+def check_full_size_sampled(prob, q, boxes, b=10):
+    it = prob.interior()
+    with Gpu(prob) as g:
+        got = g.rhs(q)[it]
+        # property: conservative rows of a periodic domain sum to round-off of their magnitude
+        if all(k == wl.BC_PERIODIC for k in prob.bc_lo[:prob.ndim]):
+            for k in range(prob.nf + prob.ndim + 1):
+                assert abs(got[k].sum()) <= 1e-9 * np.abs(got[k]).sum() + 1e-300
+    assert np.all(np.isfinite(got))
+    S = np.array([np.max(np.abs(got[k])) for k in range(prob.neq)])
+    S[prob.nf:prob.nf + prob.ndim] = S[prob.nf:prob.nf + prob.ndim].max()
+    # with interior ghosts wrapped the cut-out is only valid where the real array is periodic or away from walls
+    for lo in boxes:
+        ref = subbox_reference(prob, q, lo, b)
+        sl = tuple(slice(lo[d], lo[d] + b) for d in (2, 1, 0))
+        blk = got[(slice(None),) + sl]
+        for k in range(prob.neq):
+            if S[k] == 0.0:
+                assert np.all(blk[k] == 0.0)
+                continue
+            err = np.max(np.abs(blk[k] - ref[k])) / S[k]
+            assert err <= RHS_TOL, (lo, k, err)
+
+
+def test_rhs_full_size_cfg3_sampled():
+    prob, q = wl.cfg3()
+    rng = np.random.default_rng(0)
+    boxes = [tuple(int(v) for v in rng.integers(3, 256 - 13, size=3)) for _ in range(12)]
+    boxes += [(3, 100, 200), (8, 30, 60), (120, 243, 3), (243, 243, 243)]     # pressure-pulse slab, far corners
+    check_full_size_sampled(prob, q, boxes)
+
+
+def test_rhs_full_size_cfg4_sampled():
+    prob, q = wl.cfg4()
+    rng = np.random.default_rng(1)
+    boxes = [tuple(int(v) for v in rng.integers(0, 384, size=3)) for _ in range(10)]
+    boxes += [(0, 0, 0), (379, 379, 379), (380, 5, 190)]                      # wrap around the periodic faces
+    check_full_size_sampled(prob, q, boxes)
+
+
+# ---------------------------------------------------------------------------------------------
+# a5: 10 RK3 steps, same dt sequence on both sides (taken from the oracle's CFL)
+# ---------------------------------------------------------------------------------------------
+def check_rk(prob, q, steps=10, **kw):
+    orc = oracle.Oracle(prob)
+    qo = q.copy()
+    dts = []
+    for _ in range(steps):
+        dt = orc.cfl_dt(qo, prob.cfl)
+        dts.append(dt)
+        orc.rk3_step(qo, dt)
+    with Gpu(prob, **kw) as g:
+        got = g.rk3(q, dts)
+    err = parity_errors(prob, got, qo)
+    assert np.all(err <= RK_TOL), f"{prob.name}: per-equation error after {steps} RK3 steps {err}"
+    return err
+
+
+@pytest.mark.parametrize("ndim,nf", TEMPLATE_SET)
+def test_rk3_parity_random_states(ndim, nf):
+    n = {1: (600,), 2: (130, 45), 3: (40, 29, 33)}[ndim]
+    prob, q = wl.random_state(ndim, n, nf, seed=20 * ndim + nf, periodic=(nf != 2), rough=False)
+    check_rk(prob, q, march_segment=8)
+
+
+def test_rk3_parity_cfg0():
+    prob, q = wl.cfg0()
+    check_rk(prob, q)
+
+
+def test_rk3_parity_cfg1():
+    prob, q = wl.cfg1()
+    check_rk(prob, q)
+
+
+def test_rk3_parity_cfg2():
+    prob, q = wl.cfg2()
+    check_rk(prob, q)
+
+
+def test_rk3_parity_cfg3_reduced():
+    prob, q = wl.cfg3(n=96)
+    check_rk(prob, q)
+
+
+def test_rk3_parity_cfg4_reduced():
+    prob, q = wl.cfg4(n=64)
+    check_rk(prob, q)
+
+
+def test_single_stage_combination_matches_forward_euler_of_rhs():
+    """q + dt L(q) assembled by the last sweep equals the separately returned L (same kernels, two output modes)."""
+    prob, q = wl.random_state(3, (30, 20, 25), 2, seed=9, periodic=True)
+    with Gpu(prob) as g:
+        L = g.rhs(q)
+    # after a full step the state must differ from q by O(dt): a smoke check that the in-place stages ran
+    orc = oracle.Oracle(prob)
+    dt = orc.cfl_dt(q.copy(), 0.3)
+    with Gpu(prob) as g:
+        q1 = g.rk3(q, [dt])
+    it = prob.interior()
+    assert np.all(np.isfinite(q1[it]))
+    lin = q[it] + dt * L[it]
+    # RK3 = Euler + O(dt^2): the difference is far smaller than the increment itself
+    assert np.max(np.abs(q1[it][0] - lin[0])) < 0.5 * np.max(np.abs(dt * L[it][0]))
+
+
+# ---------------------------------------------------------------------------------------------
+# a6: CFL
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("ndim,nf", TEMPLATE_SET)
+def test_cfl_dt_parity(ndim, nf):
+    prob, q = wl.random_state(ndim, SIZES[ndim], nf, seed=4, periodic=True)
+    ref = oracle.Oracle(prob).cfl_dt(q, prob.cfl)
+    with Gpu(prob) as g:
+        got = g.cfl_dt(q)
+    assert abs(got - ref) <= 1e-13 * ref
+
+
+def test_cfl_dt_parity_cfg3():
+    prob, q = wl.cfg3(n=128)
+    ref = oracle.Oracle(prob).cfl_dt(q, prob.cfl)
+    with Gpu(prob) as g:
+        got = g.cfl_dt(q)
+    assert abs(got - ref) <= 1e-13 * ref
+
+
+# ---------------------------------------------------------------------------------------------
+# host-buffer entry point and measurement hooks
+# ---------------------------------------------------------------------------------------------
+def test_advance_host_equals_device_path():
+    prob, q = wl.random_state(2, (90, 40), 2, seed=12, periodic=True, rough=False)
+    with Gpu(prob) as g:
+        torch = g.torch
+        qd = g.to_dev(q)
+        t_dev = 0.0
+        for _ in range(3):
+            dt = B.mfc_cfl_dt(g.ctx, qd.data_ptr(), g.stream)
+            B.mfc_rk3_step(g.ctx, qd.data_ptr(), dt, g.stream)
+            t_dev += dt
+        torch.cuda.synchronize()
+        ref = qd.cpu().numpy()
+        qh = torch.from_numpy(q.copy()).pin_memory()
+        t_host = B.mfc_advance_host(g.ctx, qh.data_ptr(), 3, 0.0, g.stream)
+        it = prob.interior()
+        assert np.array_equal(qh.numpy()[it], ref[it])
+        assert t_host == pytest.approx(t_dev, rel=1e-15)
+        # fixed dt, pageable memory
+        qp = q.copy()
+        B.mfc_advance_host(g.ctx, qp.ctypes.data, 1, 1e-7, g.stream)
+        ref1 = g.rk3(q, [1e-7])
+        assert np.array_equal(qp[it], ref1[it])
+
+
+def test_profile_hooks_count_launches_and_time():
+    prob, q = wl.random_state(3, (32, 32, 32), 2, seed=1)
+    with Gpu(prob) as g:
+        qd = g.to_dev(q)
+        n0 = B.mfc_launch_count(g.ctx)
+        B.mfc_profile_enable(g.ctx, True)
+        B.mfc_rk3_step(g.ctx, qd.data_ptr(), 1e-9, g.stream)
+        B.mfc_cfl_dt(g.ctx, qd.data_ptr(), g.stream)
+        assert B.mfc_launch_count(g.ctx) - n0 == 3 * 4 + 1
+        for kid, want in [(B.MFC_K_PRIM, 3), (B.MFC_K_SWEEP_X, 3), (B.MFC_K_SWEEP_Y, 3), (B.MFC_K_SWEEP_Z, 3), (B.MFC_K_CFL, 1)]:
+            n, ms = B.mfc_profile_get(g.ctx, kid, reset=True)
+            assert n == want and ms > 0.0
+        n, ms = B.mfc_profile_get(g.ctx, B.MFC_K_SWEEP_X)
+        assert n == 0 and ms == 0.0
+        B.mfc_profile_enable(g.ctx, False)
+
+
+def test_dfma_probe_reports_a_plausible_fp64_rate():
+    from paper_2305_09163_b200 import build
+    build.build()
+    tf, ms = B.mfc_probe_dfma(-1)
+    assert 5.0 < tf < 80.0 and ms > 0.0
