@@ -80,23 +80,59 @@ class Gpu:
         return vL.cpu().numpy(), vR.cpu().numpy(), F.cpu().numpy(), uf.cpu().numpy()
 
 
-def row_scales(prob, ref_int: np.ndarray, alpha_floor: float = 0.0) -> np.ndarray:
-    """S_k = max |ref_k| over the interior; the D momentum rows share one scale (a transverse momentum RHS can be
-    pure cancellation noise); alpha rows are floored (an alpha RHS can vanish identically)."""
+EPS_MACH = 2.0 ** -52
+RHS_TOL = 1.0e-10
+ROUNDOFF_K = 32.0          # "a few ulp": rounding errors accumulated by one face flux, DESIGN.md "Parity norm"
+
+
+def rhs_floors(prob, orc, q: np.ndarray) -> np.ndarray:
+    """Round-off floors of the per-equation RHS scales, from oracle quantities only.
+
+    Two correct fp64 evaluations of one face flux differ by a few ulp of every reconstructed state.  The face
+    velocity u_face is built from u -/+ c and p/(rho c), so it carries an absolute error of a few eps * lam,
+    lam = max(|u| + c), however small u_face itself is.  Each flux row inherits it at its own flux scale
+        alpha_i rho_i : max(alpha_i rho_i) lam       alpha_i : max(alpha_i) lam
+        rho u_d       : max|p| + max(rho) lam max|u| (acoustic coupling rho c du)
+        rho E         : max|E + p| lam
+    and the RHS at that scale / dx, whatever the magnitude of the RHS itself (which can vanish identically: a
+    quiescent bubble, a transverse momentum row).  S_k is floored at K eps / tol times that scale, K = 32, so
+    that `tol relative` never asks for less than K ulp of the flux terms that cancel.
+    """
+    it = prob.interior()
+    w = orc.cons_to_prim(q)[it]
+    nf, D = prob.nf, prob.ndim
+    dxmin, dxmax = min(prob.dx[:D]), max(prob.dx[:D])
+    lam = dxmax / orc.cfl_dt(q, 1.0)                           # >= max_d max_cells (|u_d| + c)
+    rho = w[:nf].sum(axis=0)
+    umax = max(float(np.max(np.abs(w[nf + d]))) for d in range(D))
+    pmax = float(np.max(np.abs(w[nf + D])))
+    F = np.zeros(prob.neq)
+    for i in range(nf):
+        F[i] = float(np.max(np.abs(w[i]))) * lam
+    F[nf:nf + D] = pmax + float(rho.max()) * lam * umax
+    F[nf + D] = float(np.max(np.abs(q[it][nf + D]) + np.abs(w[nf + D]))) * lam
+    for k in range(nf + D + 1, prob.neq):
+        F[k] = float(np.max(np.abs(w[k]))) * lam
+    return ROUNDOFF_K * EPS_MACH / RHS_TOL * F / dxmin
+
+
+def row_scales(prob, ref_int: np.ndarray, floors=None) -> np.ndarray:
+    """S_k = max(max |ref_k| over the interior, floor_k); the D momentum rows share one scale (a transverse
+    momentum RHS can be pure cancellation noise)."""
     nf, D = prob.nf, prob.ndim
     S = np.array([np.max(np.abs(ref_int[k])) for k in range(prob.neq)])
     S[nf:nf + D] = S[nf:nf + D].max()
-    for k in range(nf + D + 1, prob.neq):
-        S[k] = max(S[k], alpha_floor)
+    if floors is not None:
+        S = np.maximum(S, floors)
     return S
 
 
-def parity_errors(prob, got: np.ndarray, ref: np.ndarray, alpha_floor: float = 0.0) -> np.ndarray:
+def parity_errors(prob, got: np.ndarray, ref: np.ndarray, floors=None) -> np.ndarray:
     """max_cells |got_k - ref_k| / S_k per equation, interior cells only."""
     it = prob.interior()
     g, r = got[it], ref[it]
     assert np.all(np.isfinite(g)), "non-finite values in the GPU result"
-    S = row_scales(prob, r, alpha_floor)
+    S = row_scales(prob, r, floors)
     err = np.zeros(prob.neq)
     for k in range(prob.neq):
         d = np.max(np.abs(g[k] - r[k]))
