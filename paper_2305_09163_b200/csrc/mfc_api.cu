@@ -1,7 +1,7 @@
 // C ABI of libmfc_b200 (include/mfc.h): context, scratch memory, the order of launches of one RHS evaluation
 // and of the 3-stage TVD Runge-Kutta step, the CFL reduction, the host-buffer entry point and the
 // measurement hooks.  No arithmetic of the method lives here: every step of the path runs in the kernels
-// of mfc_device.cuh.  No CPU fallback.
+// of mfc_kernels.cuh.  No CPU fallback.
 #include "../../include/mfc.h"
 #include "mfc_launch.h"
 
@@ -78,7 +78,7 @@ struct mfc_ctx {
     long long elems = 0;
     mfc::Geo g{};
     mfc::Eos e{};
-    double *w = nullptr, *q1 = nullptr, *acc = nullptr, *q_own = nullptr;
+    double *w = nullptr, *q1 = nullptr, *q_own = nullptr;
     unsigned long long *min_dev = nullptr;
     unsigned long long *min_host = nullptr;  // pinned
     bool profile = false;
@@ -152,8 +152,9 @@ int cuda_to_status(cudaError_t e)
     return MFC_ECUDA;
 }
 
-// One evaluation of L on the primitive array built from q_in; `fin` describes what the last sweep emits.
-int eval_L(mfc_ctx *c, const double *q_in, double *acc, SweepOut fin, cudaStream_t s)
+// One evaluation of L on the primitive array built from q_in.  The x sweep writes out = base + coef L_x (base
+// described by `o`), the y and z sweeps add coef L_y, coef L_z in place (SweepOut, mfc_launch.h).
+int eval_L(mfc_ctx *c, const double *q_in, SweepOut o, cudaStream_t s)
 {
     cudaError_t err;
     {
@@ -162,12 +163,7 @@ int eval_L(mfc_ctx *c, const double *q_in, double *acc, SweepOut fin, cudaStream
     }
     if (err != cudaSuccess) return cuda_to_status(err);
     for (int dir = 0; dir < c->ndim; ++dir) {
-        SweepOut o = fin;
-        if (dir != c->ndim - 1) {
-            o.rk = 0;
-            o.acc_out = acc;
-        }
-        o.acc_in = dir == 0 ? nullptr : acc;
+        o.first = dir == 0;
         {
             Timed t(c, MFC_K_SWEEP_X + dir, s);
             err = launch_sweep(c->ndim, c->nf, dir, c->g, c->e, c->w, o, c->segment, s);
@@ -177,22 +173,22 @@ int eval_L(mfc_ctx *c, const double *q_in, double *acc, SweepOut fin, cudaStream
     return MFC_OK;
 }
 
+// 3-stage TVD Runge-Kutta.  Every stage is out = ca qn + cb (qs + dt L(qs)); the sweeps read the
+// primitive array, and each cell's qs / qn / out are touched by one thread, so stages 2 and 3 run in place.
 int rk3(mfc_ctx *c, double *q, double dt, cudaStream_t s)
 {
     SweepOut f{};
-    f.rk = 1;
-    f.dt = dt;
     // q1 = q + dt L(q)
-    f.qn = q; f.qs = q; f.out = c->q1; f.ca = 0.0; f.cb = 1.0;
-    int st = eval_L(c, q, c->acc, f, s);
+    f.out = c->q1; f.qs = q; f.qn = q; f.ca = 0.0; f.cb = 1.0; f.coef = dt; f.nbase = 1;
+    int st = eval_L(c, q, f, s);
     if (st) return st;
-    // q2 = 3/4 q + 1/4 (q1 + dt L(q1)), in place over q1 (the sweeps read the primitive array, not q1)
-    f.qn = q; f.qs = c->q1; f.out = c->q1; f.ca = 0.75; f.cb = 0.25;
-    st = eval_L(c, c->q1, c->acc, f, s);
+    // q2 = 3/4 q + 1/4 (q1 + dt L(q1)), in place over q1
+    f.out = c->q1; f.qs = c->q1; f.qn = q; f.ca = 0.75; f.cb = 0.25; f.coef = 0.25 * dt; f.nbase = 2;
+    st = eval_L(c, c->q1, f, s);
     if (st) return st;
     // q <- 1/3 q + 2/3 (q2 + dt L(q2))
-    f.qn = q; f.qs = c->q1; f.out = q; f.ca = 1.0 / 3.0; f.cb = 2.0 / 3.0;
-    return eval_L(c, c->q1, c->acc, f, s);
+    f.out = q; f.qs = c->q1; f.qn = q; f.ca = 1.0 / 3.0; f.cb = 2.0 / 3.0; f.coef = (2.0 / 3.0) * dt; f.nbase = 2;
+    return eval_L(c, c->q1, f, s);
 }
 
 int cfl_dt(mfc_ctx *c, const double *q, double *dt_host, cudaStream_t s)
@@ -324,10 +320,10 @@ int mfc_init(mfc_ctx **out, const mfc_grid *grid, int n_fluids, const mfc_fluid 
     }
 
     DeviceGuard guard(dev);
+    if (cudaDeviceGetAttribute(&g.sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) g.sms = 0;
     const size_t bytes = (size_t)c->elems * sizeof(double);
     cudaError_t err = cudaMalloc((void **)&c->w, bytes);
     if (err == cudaSuccess) err = cudaMalloc((void **)&c->q1, bytes);
-    if (err == cudaSuccess) err = cudaMalloc((void **)&c->acc, bytes);
     if (err == cudaSuccess) err = cudaMalloc((void **)&c->min_dev, sizeof(unsigned long long));
     if (err == cudaSuccess) err = cudaMallocHost((void **)&c->min_host, sizeof(unsigned long long));
     if (err != cudaSuccess) {
@@ -349,7 +345,6 @@ void mfc_destroy(mfc_ctx *c)
         for (cudaEvent_t ev : c->pool) cudaEventDestroy(ev);
         cudaFree(c->w);
         cudaFree(c->q1);
-        cudaFree(c->acc);
         cudaFree(c->q_own);
         cudaFree(c->min_dev);
         if (c->min_host) cudaFreeHost(c->min_host);
@@ -373,9 +368,8 @@ int mfc_rhs(mfc_ctx *c, const double *q_dev, double *rhs_dev, void *stream)
     if (!c || !q_dev || !rhs_dev || q_dev == rhs_dev) return MFC_EINVAL;
     DeviceGuard guard(c->device);
     SweepOut f{};
-    f.rk = 0;
-    f.acc_out = rhs_dev;
-    return eval_L(c, q_dev, rhs_dev, f, (cudaStream_t)stream);
+    f.out = rhs_dev; f.coef = 1.0; f.nbase = 0;
+    return eval_L(c, q_dev, f, (cudaStream_t)stream);
 }
 
 int mfc_rk3_step(mfc_ctx *c, double *q_dev, double dt, void *stream)

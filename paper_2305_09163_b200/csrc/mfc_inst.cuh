@@ -1,6 +1,6 @@
 // Launchers of every kernel family for one value of D (= MFC_D, set by the including translation unit), all
 // NF in {1,2,3}.  One translation unit per D keeps the sm_100a compile parallel.
-#include "mfc_device.cuh"
+#include "mfc_kernels.cuh"
 
 #ifndef MFC_D
 #error "define MFC_D (1, 2 or 3) before including mfc_inst.cuh"
@@ -26,16 +26,32 @@ cudaError_t MFC_CAT(launch_prim_d, MFC_D)(int nf, const Geo &g, const Eos &e, co
     return cudaGetLastError();
 }
 
+template <int D, int NF>
+static void launch_x(const Geo &g, const Eos &e, const double *w, const SweepOut &o, cudaStream_t s)
+{
+    constexpr int NEQ = 2 * NF + D;
+    constexpr int bytes = sweep_x_smem_bytes<NEQ>();
+    const long long G = (long long)g.n[1] * g.n[2] * g.p[0];
+    const long long ntiles = (G - 2 * NG + (XT - 2) - 1) / (XT - 2);
+    const long long cap = 2LL * (g.sms > 0 ? g.sms : 148);            // two resident blocks per multiprocessor
+    const unsigned blocks = (unsigned)(ntiles < cap ? ntiles : cap);
+    cudaFuncSetAttribute(sweep_x_kernel<D, NF>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    sweep_x_kernel<D, NF><<<blocks, XT, bytes, s>>>(g, e, w, o, (int)ntiles);
+}
+
 template <int D, int NF, int DIR>
 static void launch_march(const Geo &g, const Eos &e, const double *w, const SweepOut &o, int segment, cudaStream_t s)
 {
     constexpr int OTH = DIR == 1 ? 2 : 1;
+    constexpr int NEQ = 2 * NF + D;
+    constexpr int bytes = sweep_march_smem_bytes<NEQ>();
     const int nm = g.n[DIR];
     const int seg = segment < 1 ? 1 : (segment > nm ? nm : segment);
     const int nseg = (nm + seg - 1) / seg;
     const long long threads = (long long)g.n[0] * g.n[OTH] * nseg;
     const unsigned blocks = (unsigned)((threads + MBT - 1) / MBT);
-    sweep_march_kernel<D, NF, DIR><<<blocks, MBT, 0, s>>>(g, e, w, o, seg, nseg);
+    cudaFuncSetAttribute(sweep_march_kernel<D, NF, DIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    sweep_march_kernel<D, NF, DIR><<<blocks, MBT, bytes, s>>>(g, e, w, o, seg, nseg);
 }
 
 cudaError_t MFC_CAT(launch_sweep_d, MFC_D)(int nf, int dir, const Geo &g, const Eos &e, const double *w, const SweepOut &o,
@@ -44,9 +60,7 @@ cudaError_t MFC_CAT(launch_sweep_d, MFC_D)(int nf, int dir, const Geo &g, const 
     constexpr int D = MFC_D;
     if (dir < 0 || dir >= D) return cudaErrorInvalidValue;
     if (dir == 0) {
-        const long long total = (long long)g.n[1] * g.n[2] * (g.n[0] + 2);
-        const unsigned blocks = (unsigned)((total - 2 + (XBT - 2) - 1) / (XBT - 2));
-        MFC_FOR_NF(nf, (sweep_x_kernel<D, NF><<<blocks, XBT, 0, s>>>(g, e, w, o)))
+        MFC_FOR_NF(nf, (launch_x<D, NF>(g, e, w, o, s)))
     }
 #if MFC_D >= 2
     else if (dir == 1) {

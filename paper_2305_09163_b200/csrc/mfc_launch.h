@@ -18,6 +18,7 @@ struct Geo {
     long long cells;     // p[0] * p[1] * p[2] : stride between equations
     double inv_dx[3];
     int bc_lo[3], bc_hi[3];
+    int sms;             // multiprocessors of the device (persistent grids are sized from it)
 };
 
 // stiffened-gas tables, PAPER.md:54-58 (Eq. 1), alpha-weighted mixture (reading B2)
@@ -30,16 +31,18 @@ struct Eos {
     double weno_eps4;    // 4 * eps : smoothness indicators are carried scaled by 4
 };
 
-// output stage of a sweep: total = (acc_in ? acc_in[cell] : 0) + this direction's contribution;
-//   rk == 0 : acc_out[cell] = total
-//   rk == 1 : out[cell] = ca * qn[cell] + cb * (qs[cell] + dt * total)
+// output stage of a sweep (a4 + a5).  L_dir = this direction's flux difference (+ alpha div u term):
+//   first == 1 (x sweep) : out[cell] = base + coef * L_dir,  base = cb * qs[cell] + ca * qn[cell]
+//                          (nbase = 0: base = 0;  nbase = 1: cb * qs only;  nbase = 2: both)
+//   first == 0 (y, z)    : out[cell] = out[cell] + coef * L_dir
+// mfc_rhs: coef = 1, nbase = 0.  RK stage: coef = cb * dt, so that after the last sweep
+//   out = ca * qn + cb * (qs + dt * L(qs)).  Each cell's qs, qn, out are touched by one thread only, so out may
+//   alias qs or qn (the stages run in place).
 struct SweepOut {
-    const double *acc_in;
-    double *acc_out;
-    const double *qn, *qs;
     double *out;
-    double ca, cb, dt;
-    int rk;
+    const double *qs, *qn;
+    double ca, cb, coef;
+    int first, nbase;
 };
 
 struct KernelTimer;  // opaque to the launchers
