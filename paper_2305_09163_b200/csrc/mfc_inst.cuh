@@ -51,6 +51,7 @@ static void launch_march(const Geo &g, const Eos &e, const double *w, const Swee
     const long long threads = (long long)g.n[0] * g.n[OTH] * nseg;
     const unsigned blocks = (unsigned)((threads + MBT - 1) / MBT);
     cudaFuncSetAttribute(sweep_march_kernel<D, NF, DIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    cudaFuncSetAttribute(sweep_march_kernel<D, NF, DIR>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
     sweep_march_kernel<D, NF, DIR><<<blocks, MBT, bytes, s>>>(g, e, w, o, seg, nseg);
 }
 

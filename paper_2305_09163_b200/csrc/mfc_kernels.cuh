@@ -158,7 +158,7 @@ constexpr int MA = 1;            // planes in flight beyond the stencil window
 constexpr int MR = 5 + MA;       // ring slots
 
 template <int NEQ>
-constexpr int sweep_march_smem_bytes() { return (MR + 1) * NEQ * MBT * (int)sizeof(double); }
+constexpr int sweep_march_smem_bytes() { return (MR + 2) * NEQ * MBT * (int)sizeof(double); }
 
 template <int D, int NF, int DIR>
 __global__ void __launch_bounds__(MBT, 4) sweep_march_kernel(Geo g, Eos eos, const double *__restrict__ w, SweepOut o,
@@ -172,6 +172,7 @@ __global__ void __launch_bounds__(MBT, 4) sweep_march_kernel(Geo g, Eos eos, con
     extern __shared__ double smem[];
     double *ring = smem + threadIdx.x;                    // [MR][NEQ][MBT], this thread's column
     double *park = ring + MR * SLOT;                      // [NEQ][MBT]: left state of the previous face
+    double *obuf = park + SLOT;                           // [NEQ][MBT]: out values of the cell about to be updated
     const int nx = g.n[0], no = g.n[OTH], nm = g.n[DIR];
     const long long gidx = (long long)blockIdx.x * MBT + threadIdx.x;
     if (gidx >= (long long)nx * no * nseg) return;        // no block-level barrier below
@@ -211,6 +212,11 @@ __global__ void __launch_bounds__(MBT, 4) sweep_march_kernel(Geo g, Eos eos, con
     int s0 = 0;                                           // ring slot of the oldest plane of the window
 #pragma unroll 1
     for (int k = j0 - 1; k <= j1; ++k, outp += sm) {
+        if (k > j0) {                                     // out values of cell k - 1, consumed at the end of this iteration
+            const double *ob = outp - sm;
+#pragma unroll
+            for (int e = 0; e < NEQ; ++e) cp_async8(obuf + e * MBT, ob + (long long)e * g.cells);
+        }
         issue_plane();                                    // into the slot the previous iteration's oldest plane left
         cp_async_wait<MA>();                              // planes k-2 .. k+2 have landed
         int sl[5];
@@ -234,12 +240,12 @@ __global__ void __launch_bounds__(MBT, 4) sweep_march_kernel(Geo g, Eos eos, con
             if (k > j0) {                                 // cell k - 1: its centre plane is the window's second slot
                 double *op = outp - sm;
                 const double du = ufp - ufm;
+                cp_async_wait<0>();                       // obuf has landed
 #pragma unroll
                 for (int e = 0; e < NEQ; ++e) {
                     double rr = Fm[e] - Fp[e];
                     if (e >= I::A) rr = fma(ring[sl[1] + e * MBT], du, rr);
-                    double *a = op + (long long)e * g.cells;
-                    *a = fma(c1, rr, *a);
+                    op[(long long)e * g.cells] = fma(c1, rr, obuf[e * MBT]);
                 }
             }
 #pragma unroll
