@@ -4,8 +4,8 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg3] [--n 256]
 
 One "step" is one pass of the whole path over the workload: the CFL reduction (mfc_cfl_dt) and one 3-stage
-TVD-RK step (mfc_rk3_step = 3 x [cons->prim + ghost fill, WENO5+HLLC sweeps in x, y, z, flux difference, stage
-combine]).  The workload is BASELINE.json configs[3] (256^3 two-fluid bubble cloud), seeded and synthetic.
+TVD-RK step (mfc_rk3_step = 3 launches of the fused kernel: ghost fill + cons->prim, WENO5+HLLC in x, y, z, flux
+difference, stage combine).  The workload is BASELINE.json configs[3] (256^3 two-fluid bubble cloud), seeded and synthetic.
 N > 1 (torchrun): independent replicas, one per GPU, no data-path collective ("replicas only", DESIGN.md);
 time is the max over ranks and the value counts the cells of all ranks.
 
@@ -106,19 +106,16 @@ def get_workload(name: str, n: int | None):
 
 
 # --------------------------------------------------------------------------------------------------------
-# algorithmic work of one sweep launch: per cell and direction
+# algorithmic work of one launch of the fused right-hand side, per cell
 # --------------------------------------------------------------------------------------------------------
-def sweep_algorithmic(prob, direction: int, rk_stage_mix: bool):
+def rhs_algorithmic(prob):
     neq, nf, D = prob.neq, prob.nf, prob.ndim
-    flops = neq * 80 + (102 if nf <= 2 else 116) + 3 * neq      # WENO5 (common-denominator form) + HLLC + flux difference
-    last = direction == D - 1
-    rd = neq                                                    # primitives, once
-    wr = neq
-    if direction > 0:
-        rd += neq                                               # accumulated RHS
-    if last and rk_stage_mix:
-        rd += neq * (1 + 2 / 3)                                 # q_s every stage, q_n in stages 2 and 3
-    return flops, 8.0 * (rd + wr)
+    # WENO5 in the common-denominator form (80 flops per variable and direction), HLLC (102 / 116 per face),
+    # flux difference (3 per equation and direction), cons->prim (25) and RK combine (4 per equation)
+    flops = D * (neq * 80 + (102 if nf <= 2 else 116) + 3 * neq) + 25 + 4 * neq
+    # compulsory bytes of an RK stage: q_s read once, result written once, q_n read in two of the three stages
+    doubles = neq * (1 + 1 + 2.0 / 3.0)
+    return flops, 8.0 * doubles
 
 
 def run_ours(args):
@@ -215,10 +212,9 @@ def run_ours(args):
         grind = ms_step * 1e6 / work
         hbm_peak, hbm_src = measured_peaks()
         fp64_tf, fp64_ms = B.mfc_probe_dfma(local)
-        # dominant kernel = the sweep family with the largest share of the step
-        sweeps = [("sweep_x", 0), ("sweep_y", 1), ("sweep_z", 2)][:prob.ndim]
-        dom, ddir = max(sweeps, key=lambda s: prof[s[0]]["ms_total"])
-        flops_cell, bytes_cell = sweep_algorithmic(prob, ddir, True)
+        # dominant kernel: the fused right-hand side (one launch per RK stage)
+        dom = "rhs_fused"
+        flops_cell, bytes_cell = rhs_algorithmic(prob)
         t_avg = prof[dom]["ms_avg"] * 1e-3
         ach_gbs = bytes_cell * prob.cells / t_avg / 1e9
         ach_tf = flops_cell * prob.cells / t_avg / 1e12
@@ -313,7 +309,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg3", choices=["cfg0", "cfg1", "cfg2", "cfg3", "cfg4"])
     ap.add_argument("--n", type=int, default=None, help="override cells per dimension (default: the config's size)")
-    ap.add_argument("--segment", type=int, default=0, help="marching segment of the y/z sweeps (0 = heuristic)")
+    ap.add_argument("--segment", type=int, default=0, help="z planes each block of the fused kernel marches (0 = heuristic)")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--cpu-n", type=int, default=128, help="cells per dimension of the cpu_baseline sample")
     ap.add_argument("--ref-n", type=int, default=96, help="cells per dimension of the --impl reference sample")

@@ -16,11 +16,11 @@
  *   mfc_layout() returns the padded extents and the element count of one such array.
  * Pointers: names ending in _dev are DEVICE pointers (e.g. a torch tensor's data_ptr()) on the device
  *   given to mfc_init; names ending in _host are HOST pointers.  The caller owns every buffer it passes;
- *   the library owns its scratch (primitive array, stage buffer, RHS accumulator, reduction workspace),
- *   allocated in mfc_init and released in mfc_destroy.
- * Boundary conditions are applied while the primitive array is built (ghost cells of the primitive array
- *   are computed from the wrapped / clamped interior cell).  Ghost cells of q are therefore
- *   never read and never written; ghost entries of rhs are unspecified.
+ *   the library owns its scratch (two Runge-Kutta stage arrays, reduction workspace), allocated in mfc_init
+ *   and released in mfc_destroy.
+ * Boundary conditions are applied while a tile of the state is staged on chip (a ghost cell is computed from
+ *   the wrapped / clamped interior cell).  Ghost cells of q are therefore never read and never
+ *   written; ghost entries of rhs are unspecified.
  * Streams: `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  All work is
  *   enqueued on it.  Only mfc_cfl_dt, mfc_advance_host, mfc_profile_get and mfc_probe_dfma synchronise.
  * Errors: every function returns MFC_OK (0) or a negative mfc_status; nothing is thrown or printed.
@@ -69,13 +69,13 @@ typedef struct {
     double weno_eps;   /* WENO-JS epsilon, Eq. 12 / Listing 1; <= 0 selects 1e-16 */
     double cfl;        /* CFL number used by mfc_cfl_dt; <= 0 selects 0.3 */
     int device;        /* CUDA device ordinal; < 0 selects the current device */
-    int march_segment; /* cells each thread marches in the y / z sweeps; <= 0 selects a heuristic */
+    int march_segment; /* planes each block of the fused kernel marches along z (3D); <= 0 selects a heuristic */
 } mfc_opts;
 
 typedef struct mfc_ctx mfc_ctx;
 
 /* Creates a context: validates (ndim, n_fluids) against the compiled template set, stores the EOS and BC
- * tables, allocates scratch (3 state-sized arrays).  eos: n_fluids entries.  opts may be NULL. */
+ * tables, allocates scratch (2 state-sized stage arrays).  eos: n_fluids entries.  opts may be NULL. */
 int mfc_init(mfc_ctx **out, const mfc_grid *grid, int n_fluids, const mfc_fluid *eos, const mfc_bc *bc,
              const mfc_opts *opts);
 
@@ -121,12 +121,11 @@ int mfc_line_fluxes(mfc_ctx *ctx, int dir, int n, const double *w_dev, double *v
 /* ---- measurement hooks ---- */
 
 typedef enum {
-    MFC_K_PRIM = 0,    /* cons->prim + ghost fill */
-    MFC_K_SWEEP_X = 1, /* fused WENO5 + HLLC + flux difference, x */
-    MFC_K_SWEEP_Y = 2,
-    MFC_K_SWEEP_Z = 3,
-    MFC_K_CFL = 4,
-    MFC_K_COUNT = 5
+    MFC_K_RHS = 0,  /* the fused right-hand side: ghost fill, cons->prim, WENO5 + HLLC in every direction,
+                       flux difference and RK stage combine in one launch */
+    MFC_K_CFL = 1,  /* CFL reduction */
+    MFC_K_PRIM = 2, /* stage output of mfc_cons_to_prim (parity tests only; not on the path) */
+    MFC_K_COUNT = 3
 } mfc_kernel_id;
 
 /* With profiling on, every kernel launch is bracketed by CUDA events on its own stream. */

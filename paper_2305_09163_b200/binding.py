@@ -16,9 +16,8 @@ LIB_PATH = _HERE / "libmfc_b200.so"
 MFC_NG = 3
 MFC_OK, MFC_EINVAL, MFC_EUNSUPPORTED, MFC_ECUDA, MFC_ENOMEM = 0, -1, -2, -3, -4
 MFC_BC_PERIODIC, MFC_BC_EXTRAP = 0, 1
-MFC_K_PRIM, MFC_K_SWEEP_X, MFC_K_SWEEP_Y, MFC_K_SWEEP_Z, MFC_K_CFL, MFC_K_COUNT = 0, 1, 2, 3, 4, 5
-KERNEL_NAMES = {MFC_K_PRIM: "prim", MFC_K_SWEEP_X: "sweep_x", MFC_K_SWEEP_Y: "sweep_y", MFC_K_SWEEP_Z: "sweep_z",
-                MFC_K_CFL: "cfl"}
+MFC_K_RHS, MFC_K_CFL, MFC_K_PRIM, MFC_K_COUNT = 0, 1, 2, 3
+KERNEL_NAMES = {MFC_K_RHS: "rhs_fused", MFC_K_CFL: "cfl", MFC_K_PRIM: "prim"}
 
 # every symbol include/mfc.h declares
 EXPORTS = [

@@ -21,13 +21,13 @@ cudaError_t launch_prim(int ndim, int nf, const Geo &g, const Eos &e, const doub
     }
     return cudaErrorInvalidValue;
 }
-cudaError_t launch_sweep(int ndim, int nf, int dir, const Geo &g, const Eos &e, const double *w, const SweepOut &o,
-                         int segment, cudaStream_t s)
+cudaError_t launch_rhs(int ndim, int nf, const Geo &g, const Eos &e, const double *q, const SweepOut &o, int segment,
+                       cudaStream_t s)
 {
     switch (ndim) {
-        case 1: return launch_sweep_d1(nf, dir, g, e, w, o, segment, s);
-        case 2: return launch_sweep_d2(nf, dir, g, e, w, o, segment, s);
-        case 3: return launch_sweep_d3(nf, dir, g, e, w, o, segment, s);
+        case 1: return launch_rhs_d1(nf, g, e, q, o, segment, s);
+        case 2: return launch_rhs_d2(nf, g, e, q, o, segment, s);
+        case 3: return launch_rhs_d3(nf, g, e, q, o, segment, s);
     }
     return cudaErrorInvalidValue;
 }
@@ -78,14 +78,14 @@ struct mfc_ctx {
     long long elems = 0;
     mfc::Geo g{};
     mfc::Eos e{};
-    double *w = nullptr, *q1 = nullptr, *q_own = nullptr;
+    double *q1 = nullptr, *q2 = nullptr, *q_own = nullptr;
     unsigned long long *min_dev = nullptr;
     unsigned long long *min_host = nullptr;  // pinned
     bool profile = false;
     std::vector<mfc::EventPair> pending;
     std::vector<cudaEvent_t> pool;
-    double ms[MFC_K_COUNT] = {0, 0, 0, 0, 0};
-    long long launches[MFC_K_COUNT] = {0, 0, 0, 0, 0};
+    double ms[MFC_K_COUNT] = {0, 0, 0};
+    long long launches[MFC_K_COUNT] = {0, 0, 0};
     long long launch_total = 0;
 };
 
@@ -152,29 +152,19 @@ int cuda_to_status(cudaError_t e)
     return MFC_ECUDA;
 }
 
-// One evaluation of L on the primitive array built from q_in.  The x sweep writes out = base + coef L_x (base
-// described by `o`), the y and z sweeps add coef L_y, coef L_z in place (SweepOut, mfc_launch.h).
-int eval_L(mfc_ctx *c, const double *q_in, SweepOut o, cudaStream_t s)
+// One evaluation of L(q_in), one launch: out = base + coef L(q_in), base described by `o` (SweepOut, mfc_launch.h).
+int eval_L(mfc_ctx *c, const double *q_in, const SweepOut &o, cudaStream_t s)
 {
     cudaError_t err;
     {
-        Timed t(c, MFC_K_PRIM, s);
-        err = launch_prim(c->ndim, c->nf, c->g, c->e, q_in, c->w, s);
+        Timed t(c, MFC_K_RHS, s);
+        err = launch_rhs(c->ndim, c->nf, c->g, c->e, q_in, o, c->segment, s);
     }
-    if (err != cudaSuccess) return cuda_to_status(err);
-    for (int dir = 0; dir < c->ndim; ++dir) {
-        o.first = dir == 0;
-        {
-            Timed t(c, MFC_K_SWEEP_X + dir, s);
-            err = launch_sweep(c->ndim, c->nf, dir, c->g, c->e, c->w, o, c->segment, s);
-        }
-        if (err != cudaSuccess) return cuda_to_status(err);
-    }
-    return MFC_OK;
+    return cuda_to_status(err);
 }
 
-// 3-stage TVD Runge-Kutta.  Every stage is out = ca qn + cb (qs + dt L(qs)); the sweeps read the
-// primitive array, and each cell's qs / qn / out are touched by one thread, so stages 2 and 3 run in place.
+// 3-stage TVD Runge-Kutta.  Every stage is out = ca qn + cb (qs + dt L(qs)).  A stage reads its
+// neighbours' cells of qs, so it never writes the array it evaluates L on: q -> q1 -> q2 -> q.
 int rk3(mfc_ctx *c, double *q, double dt, cudaStream_t s)
 {
     SweepOut f{};
@@ -182,13 +172,13 @@ int rk3(mfc_ctx *c, double *q, double dt, cudaStream_t s)
     f.out = c->q1; f.qs = q; f.qn = q; f.ca = 0.0; f.cb = 1.0; f.coef = dt; f.nbase = 1;
     int st = eval_L(c, q, f, s);
     if (st) return st;
-    // q2 = 3/4 q + 1/4 (q1 + dt L(q1)), in place over q1
-    f.out = c->q1; f.qs = c->q1; f.qn = q; f.ca = 0.75; f.cb = 0.25; f.coef = 0.25 * dt; f.nbase = 2;
+    // q2 = 3/4 q + 1/4 (q1 + dt L(q1))
+    f.out = c->q2; f.qs = c->q1; f.qn = q; f.ca = 0.75; f.cb = 0.25; f.coef = 0.25 * dt; f.nbase = 2;
     st = eval_L(c, c->q1, f, s);
     if (st) return st;
     // q <- 1/3 q + 2/3 (q2 + dt L(q2))
-    f.out = q; f.qs = c->q1; f.qn = q; f.ca = 1.0 / 3.0; f.cb = 2.0 / 3.0; f.coef = (2.0 / 3.0) * dt; f.nbase = 2;
-    return eval_L(c, c->q1, f, s);
+    f.out = q; f.qs = c->q2; f.qn = q; f.ca = 1.0 / 3.0; f.cb = 2.0 / 3.0; f.coef = (2.0 / 3.0) * dt; f.nbase = 2;
+    return eval_L(c, c->q2, f, s);
 }
 
 int cfl_dt(mfc_ctx *c, const double *q, double *dt_host, cudaStream_t s)
@@ -304,26 +294,13 @@ int mfc_init(mfc_ctx **out, const mfc_grid *grid, int n_fluids, const mfc_fluid 
     }
     e.weno_eps4 = 4.0 * eps;
 
-    // marching segment: enough threads for ~6 waves of 148 SMs x 256 resident threads, at least 32 cells
-    if (opts && opts->march_segment > 0) {
-        c->segment = opts->march_segment;
-    } else {
-        int seg = 1 << 30;
-        for (int dir = 1; dir < g.ndim; ++dir) {
-            const long long lines = (long long)g.n[0] * g.n[dir == 1 ? 2 : 1];
-            const long long want = (6LL * 148 * 256 + lines - 1) / lines;
-            int s = (int)((g.n[dir] + want - 1) / want);
-            if (s < 32) s = 32;
-            if (s < seg) seg = s;
-        }
-        c->segment = seg;
-    }
+    c->segment = (opts && opts->march_segment > 0) ? opts->march_segment : 0;   // 0: the launcher's heuristic
 
     DeviceGuard guard(dev);
     if (cudaDeviceGetAttribute(&g.sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) g.sms = 0;
     const size_t bytes = (size_t)c->elems * sizeof(double);
-    cudaError_t err = cudaMalloc((void **)&c->w, bytes);
-    if (err == cudaSuccess) err = cudaMalloc((void **)&c->q1, bytes);
+    cudaError_t err = cudaMalloc((void **)&c->q1, bytes);
+    if (err == cudaSuccess) err = cudaMalloc((void **)&c->q2, bytes);
     if (err == cudaSuccess) err = cudaMalloc((void **)&c->min_dev, sizeof(unsigned long long));
     if (err == cudaSuccess) err = cudaMallocHost((void **)&c->min_host, sizeof(unsigned long long));
     if (err != cudaSuccess) {
@@ -343,8 +320,8 @@ void mfc_destroy(mfc_ctx *c)
         DeviceGuard guard(c->device);
         flush_events(c);
         for (cudaEvent_t ev : c->pool) cudaEventDestroy(ev);
-        cudaFree(c->w);
         cudaFree(c->q1);
+        cudaFree(c->q2);
         cudaFree(c->q_own);
         cudaFree(c->min_dev);
         if (c->min_host) cudaFreeHost(c->min_host);

@@ -1,6 +1,7 @@
 // Launchers of every kernel family for one value of D (= MFC_D, set by the including translation unit), all
 // NF in {1,2,3}.  One translation unit per D keeps the sm_100a compile parallel.
 #include "mfc_kernels.cuh"
+#include "mfc_fused.cuh"
 
 #ifndef MFC_D
 #error "define MFC_D (1, 2 or 3) before including mfc_inst.cuh"
@@ -26,53 +27,55 @@ cudaError_t MFC_CAT(launch_prim_d, MFC_D)(int nf, const Geo &g, const Eos &e, co
     return cudaGetLastError();
 }
 
+// tile height of the fused kernel: the largest that fits the shared memory of one multiprocessor
 template <int D, int NF>
-static void launch_x(const Geo &g, const Eos &e, const double *w, const SweepOut &o, cudaStream_t s)
+constexpr int fused_ty()
 {
-    constexpr int NEQ = 2 * NF + D;
-    constexpr int bytes = sweep_x_smem_bytes<NEQ>();
-    const long long G = (long long)g.n[1] * g.n[2] * g.p[0];
-    const long long ntiles = (G - 2 * NG + (XT - 2) - 1) / (XT - 2);
-    const long long cap = 2LL * (g.sms > 0 ? g.sms : 148);            // two resident blocks per multiprocessor
-    const unsigned blocks = (unsigned)(ntiles < cap ? ntiles : cap);
-    cudaFuncSetAttribute(sweep_x_kernel<D, NF>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-    sweep_x_kernel<D, NF><<<blocks, XT, bytes, s>>>(g, e, w, o, (int)ntiles);
+    if (D == 1) return 1;
+    if (D == 2) return 8;
+    return FusedCfg<D, NF, 16>::bytes <= 227 * 1024 ? 16 : 12;
 }
 
-template <int D, int NF, int DIR>
-static void launch_march(const Geo &g, const Eos &e, const double *w, const SweepOut &o, int segment, cudaStream_t s)
+// z segment of the fused kernel: blocks = tiles * nseg should fill whole waves of the multiprocessors, and every
+// segment pays for 6 extra planes of load + cons->prim + z reconstruction (about 2 full planes of work)
+static int fused_segment(const Geo &g, long long tiles, int wanted)
 {
-    constexpr int OTH = DIR == 1 ? 2 : 1;
-    constexpr int NEQ = 2 * NF + D;
-    constexpr int bytes = sweep_march_smem_bytes<NEQ>();
-    const int nm = g.n[DIR];
-    const int seg = segment < 1 ? 1 : (segment > nm ? nm : segment);
-    const int nseg = (nm + seg - 1) / seg;
-    const long long threads = (long long)g.n[0] * g.n[OTH] * nseg;
-    const unsigned blocks = (unsigned)((threads + MBT - 1) / MBT);
-    cudaFuncSetAttribute(sweep_march_kernel<D, NF, DIR>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-    cudaFuncSetAttribute(sweep_march_kernel<D, NF, DIR>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-    sweep_march_kernel<D, NF, DIR><<<blocks, MBT, bytes, s>>>(g, e, w, o, seg, nseg);
+    const int nz = g.n[2];
+    if (wanted > 0) return wanted < nz ? wanted : nz;
+    const long long sms = g.sms > 0 ? g.sms : 148;
+    double best = 1e300;
+    int best_seg = nz;
+    for (int nseg = 1; nseg <= (nz + 3) / 4; ++nseg) {
+        const int seg = (nz + nseg - 1) / nseg;
+        const long long blocks = tiles * ((nz + seg - 1) / seg);
+        const double cost = (double)((blocks + sms - 1) / sms) * (seg + 2.0);
+        if (cost < best) { best = cost; best_seg = seg; }
+    }
+    return best_seg;
 }
 
-cudaError_t MFC_CAT(launch_sweep_d, MFC_D)(int nf, int dir, const Geo &g, const Eos &e, const double *w, const SweepOut &o,
-                                           int segment, cudaStream_t s)
+template <int D, int NF>
+static void launch_fused(const Geo &g, const Eos &e, const double *q, const SweepOut &o, int segment, cudaStream_t s)
+{
+    constexpr int TY = fused_ty<D, NF>();
+    using C = FusedCfg<D, NF, TY>;
+    static_assert(C::bytes <= 227 * 1024, "fused tile does not fit shared memory");
+    const int ntx = (g.n[0] + FTX - 1) / FTX;
+    const int nty = D >= 2 ? (g.n[1] + TY - 1) / TY : 1;
+    int seg = 1, nseg = 1;
+    if (D == 3) {
+        seg = fused_segment(g, (long long)ntx * nty, segment);
+        nseg = (g.n[2] + seg - 1) / seg;
+    }
+    cudaFuncSetAttribute(rhs_fused_kernel<D, NF, TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::bytes);
+    rhs_fused_kernel<D, NF, TY><<<(unsigned)((long long)ntx * nty * nseg), C::NT, C::bytes, s>>>(g, e, q, o, ntx, nty, seg);
+}
+
+cudaError_t MFC_CAT(launch_rhs_d, MFC_D)(int nf, const Geo &g, const Eos &e, const double *q, const SweepOut &o, int segment,
+                                         cudaStream_t s)
 {
     constexpr int D = MFC_D;
-    if (dir < 0 || dir >= D) return cudaErrorInvalidValue;
-    if (dir == 0) {
-        MFC_FOR_NF(nf, (launch_x<D, NF>(g, e, w, o, s)))
-    }
-#if MFC_D >= 2
-    else if (dir == 1) {
-        MFC_FOR_NF(nf, (launch_march<D, NF, 1>(g, e, w, o, segment, s)))
-    }
-#endif
-#if MFC_D >= 3
-    else if (dir == 2) {
-        MFC_FOR_NF(nf, (launch_march<D, NF, 2>(g, e, w, o, segment, s)))
-    }
-#endif
+    MFC_FOR_NF(nf, (launch_fused<D, NF>(g, e, q, o, segment, s)))
     return cudaGetLastError();
 }
 

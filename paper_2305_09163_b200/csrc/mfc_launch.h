@@ -31,25 +31,23 @@ struct Eos {
     double weno_eps4;    // 4 * eps : smoothness indicators are carried scaled by 4
 };
 
-// output stage of a sweep (a4 + a5).  L_dir = this direction's flux difference (+ alpha div u term):
-//   first == 1 (x sweep) : out[cell] = base + coef * L_dir,  base = cb * qs[cell] + ca * qn[cell]
-//                          (nbase = 0: base = 0;  nbase = 1: cb * qs only;  nbase = 2: both)
-//   first == 0 (y, z)    : out[cell] = out[cell] + coef * L_dir
-// mfc_rhs: coef = 1, nbase = 0.  RK stage: coef = cb * dt, so that after the last sweep
-//   out = ca * qn + cb * (qs + dt * L(qs)).  Each cell's qs, qn, out are touched by one thread only, so out may
-//   alias qs or qn (the stages run in place).
+// output stage of one evaluation of L (a4 + a5):
+//   out[cell] = base + coef * L(q)[cell],  base = cb * qs[cell] + ca * qn[cell]
+//               (nbase = 0: base = 0;  nbase = 1: cb * qs only;  nbase = 2: both)
+// mfc_rhs: coef = 1, nbase = 0.  RK stage: coef = cb * dt, so that
+//   out = ca * qn + cb * (qs + dt * L(qs)).
+// out must not alias the array L is evaluated on (blocks read their neighbours' cells of it as halo); it may
+// alias qn, whose cell is read by the thread that writes it.
 struct SweepOut {
     double *out;
     const double *qs, *qn;
     double ca, cb, coef;
-    int first, nbase;
+    int nbase;
 };
 
-struct KernelTimer;  // opaque to the launchers
-
 cudaError_t launch_prim(int ndim, int nf, const Geo &g, const Eos &e, const double *q, double *w, cudaStream_t s);
-cudaError_t launch_sweep(int ndim, int nf, int dir, const Geo &g, const Eos &e, const double *w, const SweepOut &o,
-                         int segment, cudaStream_t s);
+cudaError_t launch_rhs(int ndim, int nf, const Geo &g, const Eos &e, const double *q, const SweepOut &o, int segment,
+                       cudaStream_t s);
 cudaError_t launch_cfl(int ndim, int nf, const Geo &g, const Eos &e, const double *q, unsigned long long *min_bits,
                        cudaStream_t s);
 cudaError_t launch_line(int ndim, int nf, int dir, const Eos &e, int n, const double *w, double *vL, double *vR,
@@ -58,8 +56,8 @@ cudaError_t launch_line(int ndim, int nf, int dir, const Eos &e, int n, const do
 // per-dimension implementations
 #define MFC_DECL_DIM(D)                                                                                               \
     cudaError_t launch_prim_d##D(int nf, const Geo &g, const Eos &e, const double *q, double *w, cudaStream_t s);     \
-    cudaError_t launch_sweep_d##D(int nf, int dir, const Geo &g, const Eos &e, const double *w, const SweepOut &o,    \
-                                  int segment, cudaStream_t s);                                                       \
+    cudaError_t launch_rhs_d##D(int nf, const Geo &g, const Eos &e, const double *q, const SweepOut &o, int segment,  \
+                                cudaStream_t s);                                                                      \
     cudaError_t launch_cfl_d##D(int nf, const Geo &g, const Eos &e, const double *q, unsigned long long *min_bits,    \
                                 cudaStream_t s);                                                                      \
     cudaError_t launch_line_d##D(int nf, int dir, const Eos &e, int n, const double *w, double *vL, double *vR,       \

@@ -18,7 +18,8 @@ pytestmark = pytest.mark.gpu
 
 RK_TOL = 1.0e-8
 TEMPLATE_SET = [(1, 1), (1, 2), (1, 3), (2, 1), (2, 2), (2, 3), (3, 1), (3, 2), (3, 3)]
-# several tiles of every kernel plus ragged tails: x blocks of 254 cells, marching segments of 8
+# several tiles of the fused kernel plus ragged tails: tiles of 32 x 16 (32 x 12 with three fluids, 32 x 8 in 2D)
+# cells, z segments of 8 planes
 SIZES = {1: (1201,), 2: (301, 45), 3: (67, 29, 41)}
 
 
@@ -169,7 +170,8 @@ def test_rhs_is_independent_of_the_marching_segment(seg):
     assert np.array_equal(got[it], ref[it])
 
 
-@pytest.mark.parametrize("ndim,n", [(1, (3,)), (2, (3, 3)), (3, (3, 3, 3)), (3, (3, 300, 4)), (2, (255, 3)), (1, (254,)), (1, (255,))])
+@pytest.mark.parametrize("ndim,n", [(1, (3,)), (2, (3, 3)), (3, (3, 3, 3)), (3, (3, 300, 4)), (2, (255, 3)), (1, (32,)), (1, (33,)), (1, (64,)),
+                                    (2, (64, 16)), (2, (65, 17)), (3, (32, 16, 8)), (3, (33, 17, 9)), (3, (31, 15, 3))])
 def test_rhs_parity_smallest_and_tile_edge_sizes(ndim, n):
     prob, q = wl.random_state(ndim, n, 2, seed=5, periodic=True, rough=False)
     check_rhs(prob, q)
@@ -384,11 +386,11 @@ def test_profile_hooks_count_launches_and_time():
         B.mfc_profile_enable(g.ctx, True)
         B.mfc_rk3_step(g.ctx, qd.data_ptr(), 1e-9, g.stream)
         B.mfc_cfl_dt(g.ctx, qd.data_ptr(), g.stream)
-        assert B.mfc_launch_count(g.ctx) - n0 == 3 * 4 + 1
-        for kid, want in [(B.MFC_K_PRIM, 3), (B.MFC_K_SWEEP_X, 3), (B.MFC_K_SWEEP_Y, 3), (B.MFC_K_SWEEP_Z, 3), (B.MFC_K_CFL, 1)]:
+        assert B.mfc_launch_count(g.ctx) - n0 == 3 + 1        # one fused launch per stage + the CFL reduction
+        for kid, want in [(B.MFC_K_RHS, 3), (B.MFC_K_CFL, 1)]:
             n, ms = B.mfc_profile_get(g.ctx, kid, reset=True)
             assert n == want and ms > 0.0
-        n, ms = B.mfc_profile_get(g.ctx, B.MFC_K_SWEEP_X)
+        n, ms = B.mfc_profile_get(g.ctx, B.MFC_K_RHS)
         assert n == 0 and ms == 0.0
         B.mfc_profile_enable(g.ctx, False)
 
