@@ -4,6 +4,7 @@
 // of mfc_kernels.cuh.  No CPU fallback.
 #include "../../include/mfc.h"
 #include "mfc_launch.h"
+#include "mfc_math.cuh"
 
 #include <cmath>
 #include <cstring>
@@ -50,6 +51,16 @@ cudaError_t launch_line(int ndim, int nf, int dir, const Eos &e, int n, const do
         case 3: return launch_line_d3(nf, dir, e, n, w, vL, vR, F, uf, s);
     }
     return cudaErrorInvalidValue;
+}
+
+__global__ void eos_seed_kernel(const double *gm1, double *ygm1, int n)
+{
+    if ((int)threadIdx.x < n) ygm1[threadIdx.x] = div_seed(gm1[threadIdx.x]);
+}
+cudaError_t launch_eos_seed(const double *gm1_dev, double *ygm1_dev, int n, cudaStream_t s)
+{
+    eos_seed_kernel<<<1, 32, 0, s>>>(gm1_dev, ygm1_dev, n);
+    return cudaGetLastError();
 }
 
 struct DeviceGuard {
@@ -303,6 +314,14 @@ int mfc_init(mfc_ctx **out, const mfc_grid *grid, int n_fluids, const mfc_fluid 
     if (err == cudaSuccess) err = cudaMalloc((void **)&c->q2, bytes);
     if (err == cudaSuccess) err = cudaMalloc((void **)&c->min_dev, sizeof(unsigned long long));
     if (err == cudaSuccess) err = cudaMallocHost((void **)&c->min_host, sizeof(unsigned long long));
+    if (err == cudaSuccess) {   // reciprocal seeds of gamma_i - 1, as the device computes them (mfc_math.cuh div_seed)
+        double *tmp = nullptr;
+        err = cudaMalloc((void **)&tmp, 2 * MAX_NF * sizeof(double));
+        if (err == cudaSuccess) err = cudaMemcpy(tmp, e.gm1, MAX_NF * sizeof(double), cudaMemcpyHostToDevice);
+        if (err == cudaSuccess) err = launch_eos_seed(tmp, tmp + MAX_NF, n_fluids, 0);
+        if (err == cudaSuccess) err = cudaMemcpy(e.ygm1, tmp + MAX_NF, MAX_NF * sizeof(double), cudaMemcpyDeviceToHost);
+        cudaFree(tmp);
+    }
     if (err != cudaSuccess) {
         const int st = cuda_to_status(err);
         cudaGetLastError();

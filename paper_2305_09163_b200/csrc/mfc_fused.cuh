@@ -16,10 +16,12 @@
 //   * z: the 5-plane window of a column is thread-private: four older planes in a shared-memory ring (R) plus
 //     the plane in P; the left state of the previous face is parked in shared memory, the previous flux stays
 //     in registers, so every cell is reconstructed once and every face solved once along the march;
-//   * the faces on the rim of the tile (x: -1/2 and right state of cell FTX; y likewise) are "halo jobs"
-//     done by the first three warps while the others start on the z direction;
-//   * the in-plane part of cell (., ., p) is written as out = base + coef (L_x + L_y) when plane p is loaded;
-//     the z part is added three planes later, when face p + 1/2 is known (the line is still in L2).
+//   * the rim of the tile (left state of face -1/2 from cell -1, right state of the face past the last cell,
+//     in x and in y) is reconstructed by the first three warps while the others start on the z direction; the
+//     rim faces themselves are solved by one warp each once the first row / lane has published its state;
+//   * the in-plane part of cell (., ., p), ca q_n + coef (L_x + L_y), is written when plane p is loaded; the z
+//     part and cb q_s are added three planes later, when face p + 1/2 is known (the line is still in L2; the
+//     loads are issued before the Riemann solve that produces the last term, so their latency is covered).
 // FP64 issue needs instruction-level parallelism rather than many warps on this part (one warp per scheduler
 // with four independent chains already reaches 92 % of the DFMA peak), so the block is 16 warps with up to
 // 128 registers each and the seven variables are reconstructed as independent chains.
@@ -40,8 +42,11 @@ struct FusedCfg {
     static constexpr int PPL = PY * FPX;                            // doubles per variable in the staged plane
     static constexpr int nP = NEQ * PPL;
     static constexpr int nX = D >= 2 ? (NEQ + 1) * NT : 0;          // y exchange: right states, then fluxes
-    static constexpr int nHx = (2 * NEQ + 1) * TY;                  // rim of the tile in x: vR[NEQ][TY], F[NEQ+1][TY]
-    static constexpr int nHy = D >= 2 ? (2 * NEQ + 1) * FTX : 0;    // rim in y
+    // rim of the tile in x, per row: vL of cell -1, vR of cell 0, vR of cell FTX, flux of lane 0; the rim flux
+    // overwrites the first two once they have been read (by the thread that writes it)
+    static constexpr int nHx = (3 * NEQ + (NEQ + 1)) * TY;
+    // rim in y, per column: vL of row -1, vR of row TY; the rim flux overwrites them likewise
+    static constexpr int nHy = D >= 2 ? 2 * NEQ * FTX : 0;
     static constexpr int nR = D == 3 ? 5 * NEQ * NT : 0;            // four ring slots + parked left state
     static constexpr int doubles = nP + nX + nHx + nHy + nR;
     static constexpr int bytes = doubles * (int)sizeof(double);
@@ -49,21 +54,6 @@ struct FusedCfg {
 };
 
 __device__ __forceinline__ void prefetch_l2(const double *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
-
-// left state of the face below cell 0 (seen from cell -1) and right state of the same face (seen from cell 0);
-// pb points at cell 0 of variable 0, st is the stride along the normal direction
-template <int NEQ>
-__device__ __forceinline__ void rim_face_states(const double *pb, int st, int ppl, double eps4, double (&vL)[NEQ], double (&vR)[NEQ])
-{
-#pragma unroll
-    for (int e = 0; e < NEQ; ++e) {
-        const double *p = pb + e * ppl;
-        const double a = p[-3 * st], b = p[-2 * st], c = p[-st], d = p[0], f = p[st], h = p[2 * st];
-        double unused;
-        weno5(c, b - a, c - b, d - c, f - d, eps4, vL[e], unused);
-        weno5(d, c - b, d - c, f - d, h - f, eps4, unused, vR[e]);
-    }
-}
 
 template <int D, int NF, int TY>
 __global__ void __launch_bounds__(FTX *TY, 1)
@@ -73,14 +63,19 @@ __global__ void __launch_bounds__(FTX *TY, 1)
     using I = Idx<D, NF>;
     constexpr int NEQ = C::NEQ, NT = C::NT, PPL = C::PPL, HY = C::HY;
     constexpr int NA1 = I::NA > 0 ? I::NA : 1;
+    constexpr int RIMW = TY - 1;                                    // warp that solves the rim faces
     extern __shared__ double sm[];
     double *const P = sm;
     double *const X = P + C::nP;
-    double *const HxR = X + C::nX;
-    double *const FxH = HxR + NEQ * TY;
-    double *const HyR = FxH + (NEQ + 1) * TY;
-    double *const FyH = HyR + (D >= 2 ? NEQ * FTX : 0);
-    double *const R = FyH + (D >= 2 ? (NEQ + 1) * FTX : 0);
+    double *const HxL = X + C::nX;                                  // [NEQ][TY]   left state of face -1/2
+    double *const ExR = HxL + NEQ * TY;                             // [NEQ][TY]   right state of face -1/2 (lane 0)
+    double *const HxR = ExR + NEQ * TY;                             // [NEQ][TY]   right state of face FTX - 1/2
+    double *const ExF = HxR + NEQ * TY;                             // [NEQ+1][TY] flux of face 1/2 (lane 0)
+    double *const FxH = HxL;                                        // [NEQ+1][TY] flux of face -1/2: over HxL, ExR[0]
+    double *const HyL = ExF + (NEQ + 1) * TY;                       // [NEQ][FTX]
+    double *const HyR = HyL + (D >= 2 ? NEQ * FTX : 0);             // [NEQ][FTX]
+    double *const FyH = HyL;                                        // [NEQ+1][FTX] over HyL, HyR[0]
+    double *const R = HyR + (D >= 2 ? NEQ * FTX : 0);
     double *const park = R + (D == 3 ? 4 * NEQ * NT : 0);
 
     const int tid = threadIdx.x, i = tid & 31, j = tid >> 5;
@@ -105,16 +100,23 @@ __global__ void __launch_bounds__(FTX *TY, 1)
         return src;
     };
     constexpr int NIT = (C::PY * FPX + NT - 1) / NT;
-    auto load_plane = [&](int p) {
+    auto load_plane = [&](int p) {                                  // every load is issued before the first conversion
+        double qc[NIT][NEQ];
 #pragma unroll
         for (int it = 0; it < NIT; ++it) {
             const int c = tid + it * NT;
             if (c < C::PY * FPX) {
                 const long long src = source(p, c);
-                double qc[NEQ], wc[NEQ];
 #pragma unroll
-                for (int e = 0; e < NEQ; ++e) qc[e] = __ldg(q + (long long)e * g.cells + src);
-                cons_to_prim_cell<D, NF>(qc, eos, wc);
+                for (int e = 0; e < NEQ; ++e) qc[it][e] = __ldg(q + (long long)e * g.cells + src);
+            }
+        }
+#pragma unroll
+        for (int it = 0; it < NIT; ++it) {
+            const int c = tid + it * NT;
+            if (c < C::PY * FPX) {
+                double wc[NEQ];
+                cons_to_prim_cell<D, NF>(qc[it], eos, wc);
 #pragma unroll
                 for (int e = 0; e < NEQ; ++e) P[e * PPL + c] = wc[e];
             }
@@ -142,18 +144,20 @@ __global__ void __launch_bounds__(FTX *TY, 1)
 #pragma unroll 1
     for (int p = pstart; p < pend; ++p) {
         const int n = p - pstart;                                   // planes loaded before this one
-        if (D == 3 && p + 1 < pend) prefetch_plane(p + 1);
+        if (D == 3 && p + 1 < pend) {
+            prefetch_plane(p + 1);
+            // q_n of the cell whose in-plane part the next iteration writes
+            if (o.nbase > 1 && active && p + 1 >= k0 && p + 1 < k1) {
+                const double *pq = o.qn + (long long)(p + 1 + NG) * g.sz + col;
+#pragma unroll
+                for (int e = 0; e < NEQ; ++e) prefetch_l2(pq + (long long)e * g.cells);
+            }
+        }
 
         // ---- z: reconstruct cell p - 2, solve face (p - 2) - 1/2, close cell p - 3 ----
         if constexpr (D == 3) if (n >= 4) {
             const int c = p - 2;
             const bool close = c > k0 && active;
-            double *const op = o.out + (long long)(c - 1 + NG) * g.sz + col;
-            double ob[NEQ];
-            if (close) {
-#pragma unroll
-                for (int e = 0; e < NEQ; ++e) ob[e] = op[(long long)e * g.cells];
-            }
             const double *const ra = R + ((n + 0) & 3) * NEQ * NT + tid;
             const double *const rb = R + ((n + 1) & 3) * NEQ * NT + tid;
             const double *const rc = R + ((n + 2) & 3) * NEQ * NT + tid;
@@ -170,6 +174,16 @@ __global__ void __launch_bounds__(FTX *TY, 1)
 #pragma unroll
             for (int e = 0; e < NEQ; ++e) park[e * NT + tid] = vL[e];
             if (c >= k0) {
+                // partial result and q_s term of the cell about to be closed: issued before the Riemann solve
+                const long long cell = (long long)(c - 1 + NG) * g.sz + col;
+                double ob[NEQ];
+                if (close) {
+#pragma unroll
+                    for (int e = 0; e < NEQ; ++e) {
+                        ob[e] = o.out[(long long)e * g.cells + cell];
+                        if (o.nbase > 0) ob[e] = fma(o.cb, __ldg(o.qs + (long long)e * g.cells + cell), ob[e]);
+                    }
+                }
                 double Fp[NEQ], ufp;
                 hllc<D, NF, 2>(vLp, vR, eos, Fp, ufp);
                 if (close) {
@@ -178,7 +192,7 @@ __global__ void __launch_bounds__(FTX *TY, 1)
                     for (int e = 0; e < NEQ; ++e) {
                         double rr = Fmz[e] - Fp[e];
                         if (e >= I::A) rr = fma(ab[e - I::A], du, rr);
-                        op[(long long)e * g.cells] = fma(cz, rr, ob[e]);
+                        o.out[(long long)e * g.cells + cell] = fma(cz, rr, ob[e]);
                     }
                 }
 #pragma unroll
@@ -189,48 +203,25 @@ __global__ void __launch_bounds__(FTX *TY, 1)
 
         const bool inplane = D < 3 || (p >= k0 && p < k1);          // block-uniform
         if (inplane) {
-            // ---- rim of the tile: faces -1/2 and right states of the cell past the last one ----
+            // ---- rim states: left state of face -1/2 (from cell -1) and right state of the face past the tile ----
             for (int job = tid; job < (D >= 2 ? 96 : 32); job += NT) {
-                if (job < 16) {
-                    if (job < TY) {
-                        double vL[NEQ], vR[NEQ], F[NEQ], uf;
-                        rim_face_states<NEQ>(P + (job + HY) * FPX + NG, 1, PPL, eos.weno_eps4, vL, vR);
-                        hllc<D, NF, 0>(vL, vR, eos, F, uf);
-#pragma unroll
-                        for (int e = 0; e < NEQ; ++e) FxH[e * TY + job] = F[e];
-                        FxH[NEQ * TY + job] = uf;
-                    }
-                } else if (job < 32) {
-                    const int r = job - 16;
-                    if (r < TY) {
-                        const double *pb = P + (r + HY) * FPX + NG + FTX;
-#pragma unroll
-                        for (int e = 0; e < NEQ; ++e) {
-                            const double *s = pb + e * PPL;
-                            double unused, v;
-                            weno5(s[0], s[-1] - s[-2], s[0] - s[-1], s[1] - s[0], s[2] - s[1], eos.weno_eps4, unused, v);
-                            HxR[e * TY + r] = v;
-                        }
-                    }
-                } else if constexpr (D >= 2) { if (job < 64) {
-                    const int cc = job - 32;
-                    double vL[NEQ], vR[NEQ], F[NEQ], uf;
-                    rim_face_states<NEQ>(P + HY * FPX + NG + cc, FPX, PPL, eos.weno_eps4, vL, vR);
-                    hllc<D, NF, 1>(vL, vR, eos, F, uf);
-#pragma unroll
-                    for (int e = 0; e < NEQ; ++e) FyH[e * FTX + cc] = F[e];
-                    FyH[NEQ * FTX + cc] = uf;
-                } else {
-                    const int cc = job - 64;
-                    const double *pb = P + (HY + TY) * FPX + NG + cc;
+                const bool inx = job < 32;
+                const int r = inx ? (job & 15) : (job & 31);
+                const bool left = inx ? job < 16 : job < 64;
+                if (!inx || r < TY) {
+                    // centre cell of the reconstruction: -1 (left) or T (right) along the normal direction
+                    const int st = inx ? 1 : FPX;
+                    const double *pb = inx ? P + (r + HY) * FPX + NG + (left ? -1 : FTX) : P + (HY + (left ? -1 : TY)) * FPX + NG + r;
+                    double *dst = inx ? (left ? HxL : HxR) + r : (left ? HyL : HyR) + r;
+                    const int ds = inx ? TY : FTX;
 #pragma unroll
                     for (int e = 0; e < NEQ; ++e) {
-                        const double *s = pb + e * PPL;
-                        double unused, v;
-                        weno5(s[0], s[-FPX] - s[-2 * FPX], s[0] - s[-FPX], s[FPX] - s[0], s[2 * FPX] - s[FPX], eos.weno_eps4, unused, v);
-                        HyR[e * FTX + cc] = v;
+                        const double *s5 = pb + e * PPL;
+                        double vl, vr;
+                        weno5(s5[0], s5[-st] - s5[-2 * st], s5[0] - s5[-st], s5[st] - s5[0], s5[2 * st] - s5[st], eos.weno_eps4, vl, vr);
+                        dst[e * ds] = left ? vl : vr;
                     }
-                } }
+                }
             }
 
             // ---- y, first half: reconstruct, publish the right state ----
@@ -239,13 +230,13 @@ __global__ void __launch_bounds__(FTX *TY, 1)
                 double vRy[NEQ];
 #pragma unroll
                 for (int e = 0; e < NEQ; ++e) {
-                    const double *s = pc + e * PPL;
-                    weno5(s[0], s[-FPX] - s[-2 * FPX], s[0] - s[-FPX], s[FPX] - s[0], s[2 * FPX] - s[FPX], eos.weno_eps4, vLy[e], vRy[e]);
+                    const double *s5 = pc + e * PPL;
+                    weno5(s5[0], s5[-FPX] - s5[-2 * FPX], s5[0] - s5[-FPX], s5[FPX] - s5[0], s5[2 * FPX] - s5[FPX], eos.weno_eps4, vLy[e], vRy[e]);
                 }
 #pragma unroll
                 for (int e = 0; e < NEQ; ++e) X[e * NT + tid] = vRy[e];
             }
-            __syncthreads();                                        // S1: rim results and y right states are visible
+            __syncthreads();                                        // S1: rim states and y right states are visible
 
             // ---- x: reconstruct, exchange by shuffles, solve face i + 1/2, difference ----
             double acc[NEQ];
@@ -253,8 +244,12 @@ __global__ void __launch_bounds__(FTX *TY, 1)
                 double vL[NEQ], vR[NEQ];
 #pragma unroll
                 for (int e = 0; e < NEQ; ++e) {
-                    const double *s = pc + e * PPL;
-                    weno5(s[0], s[-1] - s[-2], s[0] - s[-1], s[1] - s[0], s[2] - s[1], eos.weno_eps4, vL[e], vR[e]);
+                    const double *s5 = pc + e * PPL;
+                    weno5(s5[0], s5[-1] - s5[-2], s5[0] - s5[-1], s5[1] - s5[0], s5[2] - s5[1], eos.weno_eps4, vL[e], vR[e]);
+                }
+                if (i == 0) {
+#pragma unroll
+                    for (int e = 0; e < NEQ; ++e) ExR[e * TY + j] = vR[e];
                 }
 #pragma unroll
                 for (int e = 0; e < NEQ; ++e) {
@@ -263,30 +258,63 @@ __global__ void __launch_bounds__(FTX *TY, 1)
                 }
                 double Fp[NEQ], ufp;
                 hllc<D, NF, 0>(vL, vR, eos, Fp, ufp);
-                double ufm = __shfl_up_sync(0xffffffffu, ufp, 1);
-                if (i == 0) ufm = FxH[NEQ * TY + j];
-                const double du = ufp - ufm;
+                if (i == 0) {
+#pragma unroll
+                    for (int e = 0; e < NEQ; ++e) ExF[e * TY + j] = Fp[e];
+                    ExF[NEQ * TY + j] = ufp;
+                }
+                const double du = ufp - __shfl_up_sync(0xffffffffu, ufp, 1);
 #pragma unroll
                 for (int e = 0; e < NEQ; ++e) {
-                    double fm = __shfl_up_sync(0xffffffffu, Fp[e], 1);
-                    if (i == 0) fm = FxH[e * TY + j];
-                    double rr = fm - Fp[e];
+                    double rr = __shfl_up_sync(0xffffffffu, Fp[e], 1) - Fp[e];
+                    if (e >= I::A) rr = fma(pc[e * PPL], du, rr);
+                    acc[e] = cx * rr;                               // lane 0 is redone below with the rim flux
+                }
+            }
+
+            // ---- y, second half: solve face j + 1/2 (and, one warp, the rim faces j = -1/2) ----
+            double Fy[NEQ > 0 ? NEQ : 1], ufy = 0.0;
+            if constexpr (D >= 2) {
+                double vRn[NEQ];
+#pragma unroll
+                for (int e = 0; e < NEQ; ++e) vRn[e] = j == TY - 1 ? HyR[e * FTX + i] : X[e * NT + tid + FTX];
+                hllc<D, NF, 1>(vLy, vRn, eos, Fy, ufy);
+                if (j == RIMW) {
+                    double hl[NEQ], hr[NEQ], F[NEQ], uf;
+#pragma unroll
+                    for (int e = 0; e < NEQ; ++e) { hl[e] = HyL[e * FTX + i]; hr[e] = X[e * NT + i]; }
+                    hllc<D, NF, 1>(hl, hr, eos, F, uf);
+#pragma unroll
+                    for (int e = 0; e < NEQ; ++e) FyH[e * FTX + i] = F[e];
+                    FyH[NEQ * FTX + i] = uf;
+                }
+            }
+            __syncthreads();                                        // S2: y right states have been read, lane-0 states are visible
+            if constexpr (D >= 2) {
+#pragma unroll
+                for (int e = 0; e < NEQ; ++e) X[e * NT + tid] = Fy[e];
+                X[NEQ * NT + tid] = ufy;
+            }
+            if (j == RIMW && i < TY) {                              // rim faces i = -1/2, one per row
+                double hl[NEQ], hr[NEQ], F[NEQ], uf;
+#pragma unroll
+                for (int e = 0; e < NEQ; ++e) { hl[e] = HxL[e * TY + i]; hr[e] = ExR[e * TY + i]; }
+                hllc<D, NF, 0>(hl, hr, eos, F, uf);
+#pragma unroll
+                for (int e = 0; e < NEQ; ++e) FxH[e * TY + i] = F[e];
+                FxH[NEQ * TY + i] = uf;
+            }
+            __syncthreads();                                        // S3: fluxes are visible
+            if (i == 0) {
+                const double du = ExF[NEQ * TY + j] - FxH[NEQ * TY + j];
+#pragma unroll
+                for (int e = 0; e < NEQ; ++e) {
+                    double rr = FxH[e * TY + j] - ExF[e * TY + j];
                     if (e >= I::A) rr = fma(pc[e * PPL], du, rr);
                     acc[e] = cx * rr;
                 }
             }
-
-            // ---- y, second half: solve face j + 1/2, exchange the flux, difference ----
             if constexpr (D >= 2) {
-                double vRn[NEQ], Fy[NEQ], ufy;
-#pragma unroll
-                for (int e = 0; e < NEQ; ++e) vRn[e] = j == TY - 1 ? HyR[e * FTX + i] : X[e * NT + tid + FTX];
-                hllc<D, NF, 1>(vLy, vRn, eos, Fy, ufy);
-                __syncthreads();                                    // S2: every right state has been read
-#pragma unroll
-                for (int e = 0; e < NEQ; ++e) X[e * NT + tid] = Fy[e];
-                X[NEQ * NT + tid] = ufy;
-                __syncthreads();                                    // S3: fluxes are visible
                 const double ufm = j == 0 ? FyH[NEQ * FTX + i] : X[NEQ * NT + tid - FTX];
                 const double du = ufy - ufm;
 #pragma unroll
@@ -298,15 +326,16 @@ __global__ void __launch_bounds__(FTX *TY, 1)
                 }
             }
 
-            // ---- a4 + a5: out = ca qn + cb qs + coef (L_x + L_y); the z part follows three planes later ----
+            // ---- a4 + a5: coef (L_x + L_y) + ca q_n now (out may be q_n itself, so q_n is read before this cell of
+            // out is first written); the z part and cb q_s follow three planes later ----
             if (active) {
                 const long long cell = (D == 3 ? (long long)(p + NG) * g.sz : 0) + col;
 #pragma unroll
                 for (int e = 0; e < NEQ; ++e) {
-                    double base = 0.0;
-                    if (o.nbase > 0) base = o.cb * o.qs[(long long)e * g.cells + cell];
-                    if (o.nbase > 1) base = fma(o.ca, o.qn[(long long)e * g.cells + cell], base);
-                    o.out[(long long)e * g.cells + cell] = base + acc[e];
+                    double v = acc[e];
+                    if (o.nbase > 1) v = fma(o.ca, o.qn[(long long)e * g.cells + cell], v);
+                    if (D < 3 && o.nbase > 0) v = fma(o.cb, o.qs[(long long)e * g.cells + cell], v);
+                    o.out[(long long)e * g.cells + cell] = v;
                 }
             }
         }

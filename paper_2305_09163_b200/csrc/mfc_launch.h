@@ -26,6 +26,7 @@ struct Eos {
     // as given / as the definition divides by: used by the cons->prim kernel, which evaluates the
     // definition term by term without contraction
     double gamma[MAX_NF], pi_inf[MAX_NF], gm1[MAX_NF];
+    double ygm1[MAX_NF]; // div_seed(gm1[i]) (mfc_math.cuh), computed on the device by launch_eos_seed
     // Gamma = G_last + sum_{i<nf-1} alpha_i dG_i ;  Pi likewise  (alpha_nf = 1 - sum alpha_i)
     double G_last, P_last, dG[MAX_NF], dP[MAX_NF];
     double weno_eps4;    // 4 * eps : smoothness indicators are carried scaled by 4
@@ -50,6 +51,7 @@ cudaError_t launch_rhs(int ndim, int nf, const Geo &g, const Eos &e, const doubl
                        cudaStream_t s);
 cudaError_t launch_cfl(int ndim, int nf, const Geo &g, const Eos &e, const double *q, unsigned long long *min_bits,
                        cudaStream_t s);
+cudaError_t launch_eos_seed(const double *gm1_dev, double *ygm1_dev, int n, cudaStream_t s);
 cudaError_t launch_line(int ndim, int nf, int dir, const Eos &e, int n, const double *w, double *vL, double *vR,
                         double *F, double *uf, cudaStream_t s);
 
