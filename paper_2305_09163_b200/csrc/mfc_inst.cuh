@@ -27,17 +27,19 @@ cudaError_t MFC_CAT(launch_prim_d, MFC_D)(int nf, const Geo &g, const Eos &e, co
     return cudaGetLastError();
 }
 
-// tile height of the fused kernel: the largest that fits the shared memory of one multiprocessor
+// tile height of the fused kernel: 3D tiles are sized so that the ring, the staging buffers and the staged plane
+// fit the 227 KB of one multiprocessor with 12 (two fluids) or 8 (three fluids) warps per block
 template <int D, int NF>
 constexpr int fused_ty()
 {
     if (D == 1) return 1;
     if (D == 2) return 8;
-    return FusedCfg<D, NF, 16>::bytes <= 227 * 1024 ? 16 : 12;
+    return NF <= 2 ? 12 : 8;
 }
 
-// z segment of the fused kernel: blocks = tiles * nseg should fill whole waves of the multiprocessors, and every
-// segment pays for 6 extra planes of load + cons->prim + z reconstruction (about 2 full planes of work)
+// z segment of the march: blocks = tiles * nseg should fill whole waves of the multiprocessors (one block per
+// multiprocessor), and every segment pays for 6 extra planes of load + cons->prim + z reconstruction (about 2
+// full planes of work)
 static int fused_segment(const Geo &g, long long tiles, int wanted)
 {
     const int nz = g.n[2];
@@ -62,13 +64,15 @@ static void launch_fused(const Geo &g, const Eos &e, const double *q, const Swee
     static_assert(C::bytes <= 227 * 1024, "fused tile does not fit shared memory");
     const int ntx = (g.n[0] + FTX - 1) / FTX;
     const int nty = D >= 2 ? (g.n[1] + TY - 1) / TY : 1;
-    int seg = 1, nseg = 1;
-    if (D == 3) {
-        seg = fused_segment(g, (long long)ntx * nty, segment);
-        nseg = (g.n[2] + seg - 1) / seg;
+    if constexpr (D == 3) {
+        const int seg = fused_segment(g, (long long)ntx * nty, segment);
+        const int nseg = (g.n[2] + seg - 1) / seg;
+        cudaFuncSetAttribute(rhs_fused_march_kernel<NF, TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::bytes);
+        rhs_fused_march_kernel<NF, TY><<<(unsigned)((long long)ntx * nty * nseg), C::NT, C::bytes, s>>>(g, e, q, o, ntx, nty, seg);
+    } else {
+        cudaFuncSetAttribute(rhs_fused_plane_kernel<D, NF, TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::bytes);
+        rhs_fused_plane_kernel<D, NF, TY><<<(unsigned)((long long)ntx * nty), C::NT, C::bytes, s>>>(g, e, q, o, ntx);
     }
-    cudaFuncSetAttribute(rhs_fused_kernel<D, NF, TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::bytes);
-    rhs_fused_kernel<D, NF, TY><<<(unsigned)((long long)ntx * nty * nseg), C::NT, C::bytes, s>>>(g, e, q, o, ntx, nty, seg);
 }
 
 cudaError_t MFC_CAT(launch_rhs_d, MFC_D)(int nf, const Geo &g, const Eos &e, const double *q, const SweepOut &o, int segment,
