@@ -23,8 +23,8 @@
 //   * the rim of the tile (left state of face -1/2 from cell -1, right state of the face past the last cell,
 //     in x and in y) is reconstructed by the first three warps; the rim faces themselves are solved by one
 //     warp once the first lane / row has published its state;
-//   * out = ca q_n + cb q_s + coef (L_x + L_y + L_z): q_s of the cell is staged by cp.async during the
-//     previous iteration, q_n (L2-prefetched one iteration ahead) is loaded before the in-plane work.
+//   * out = ca q_n + cb q_s + coef (L_x + L_y + L_z): q_s of the cell is staged by cp.async at the top of the
+//     iteration, q_n (L2-prefetched one iteration ahead) is loaded at the start of the in-plane work.
 // Every global read is therefore issued long before its first use, by the thread that uses it: no block
 // barrier is involved in the staging, only cp.async.wait_group.
 // FP64 issue needs instruction-level parallelism rather than many warps on this part (one warp per scheduler
@@ -92,29 +92,42 @@ struct InplaneBufs {
 // a2 + a3 + a4 in x and y on the plane staged in P:  acc[e] += cx L_x + cy L_y  for the thread's cell.
 // Called by every thread of the block (it contains three block barriers).
 // ---------------------------------------------------------------------------------------------------------
-template <int D, int NF, int TY>
+struct NoHook {
+    __device__ __forceinline__ void operator()() const {}
+};
+
+// `early` runs at the top of the first FP64-heavy block and `mid` at the top of the second: the caller's loads,
+// cp.async issues and the cons->prim chains of the NEXT plane go there, so that they overlap this plane's
+// arithmetic instead of forming latency-bound phases of their own.
+template <int D, int NF, int TY, class Early = NoHook, class Mid = NoHook>
 __device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, const Eos &eos, double cx, double cy,
-                                           double (&acc)[2 * NF + D])
+                                           double (&acc)[2 * NF + D], Early early = Early(), Mid mid = Mid())
 {
     using C = FusedCfg<D, NF, TY>;
     using I = Idx<D, NF>;
     constexpr int NEQ = C::NEQ, NT = C::NT, PPL = C::PPL, HY = C::HY;
-    constexpr int RIMW = TY - 1;                                    // warp that solves the rim faces
+    constexpr int RIMW = TY - 1;                                    // warp that solves the y rim faces
+    constexpr int RIMX = TY >= 2 ? TY - 2 : 0;                      // warp that solves the x rim faces
     const int tid = threadIdx.x, i = tid & 31, j = tid >> 5;
     const double *const P = B.P;
     const double *const pc = P + (j + HY) * FPX + (i + NG);         // this thread's cell
     double *const FxH = B.HxL;                                      // [NEQ+1][TY]  flux of face -1/2, over HxL, ExR[0]
     double *const FyH = B.HyL;                                      // [NEQ+1][FTX] over HyL, HyR[0]
 
-    // ---- rim states: left state of face -1/2 (from cell -1) and right state of the face past the tile ----
-    for (int job = tid; job < (D >= 2 ? 96 : 32); job += NT) {
-        const bool inx = job < 32;
+    early();
+    // ---- rim states, one job per thread of the first warps: [0,16) left state of x face -1/2 (from cell -1),
+    // [16,32) right state of the x face past the tile, [32,64) / [64,96) the same in y, [96,112) right state of
+    // x face -1/2 (from cell 0: recomputed here so that the rim face can be solved before lane 0 publishes it) ----
+    for (int job = tid; job < 112; job += NT) {
+        const bool inx = job < 32 || job >= 96;
+        if (!inx && D < 2) continue;
         const int r = inx ? (job & 15) : (job & 31);
-        const bool left = inx ? job < 16 : job < 64;
+        const bool left = inx ? job < 16 : job < 64;                // which side of the cell the state is taken from
         if (!inx || r < TY) {
             const int st = inx ? 1 : FPX;                           // stride along the normal direction
-            const double *pb = inx ? P + (r + HY) * FPX + NG + (left ? -1 : FTX) : P + (HY + (left ? -1 : TY)) * FPX + NG + r;
-            double *dst = inx ? (left ? B.HxL : B.HxR) + r : (left ? B.HyL : B.HyR) + r;
+            const int cc = job >= 96 ? 0 : (left ? -1 : (inx ? FTX : TY));   // centre cell along the normal direction
+            const double *pb = inx ? P + (r + HY) * FPX + NG + cc : P + (HY + cc) * FPX + NG + r;
+            double *dst = inx ? (job >= 96 ? B.ExR : (left ? B.HxL : B.HxR)) + r : (left ? B.HyL : B.HyR) + r;
             const int ds = inx ? TY : FTX;
 #pragma unroll
             for (int e = 0; e < NEQ; ++e) {
@@ -141,6 +154,7 @@ __device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, cons
     __syncthreads();                                                // S1: rim states and y right states are visible
 
     // ---- x: reconstruct, exchange by shuffles, solve face i + 1/2, difference ----
+    mid();
     double ax[NEQ];
     {
         double vL[NEQ], vR[NEQ];
@@ -148,10 +162,6 @@ __device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, cons
         for (int e = 0; e < NEQ; ++e) {
             const double *s5 = pc + e * PPL;
             weno5(s5[0], s5[-1] - s5[-2], s5[0] - s5[-1], s5[1] - s5[0], s5[2] - s5[1], eos.weno_eps4, vL[e], vR[e]);
-        }
-        if (i == 0) {
-#pragma unroll
-            for (int e = 0; e < NEQ; ++e) B.ExR[e * TY + j] = vR[e];
         }
 #pragma unroll
         for (int e = 0; e < NEQ; ++e) {
@@ -191,13 +201,7 @@ __device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, cons
             FyH[NEQ * FTX + i] = uf;
         }
     }
-    __syncthreads();                                                // S2: y right states have been read, lane-0 states are visible
-    if constexpr (D >= 2) {
-#pragma unroll
-        for (int e = 0; e < NEQ; ++e) B.X[e * NT + tid] = Fy[e];
-        B.X8[tid] = ufy;
-    }
-    if (j == RIMW && i < TY) {                                      // rim faces i = -1/2, one per row
+    if (j == RIMX && i < TY) {                                      // rim faces i = -1/2, one per row
         double hl[NEQ], hr[NEQ], F[NEQ], uf;
 #pragma unroll
         for (int e = 0; e < NEQ; ++e) { hl[e] = B.HxL[e * TY + i]; hr[e] = B.ExR[e * TY + i]; }
@@ -205,6 +209,12 @@ __device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, cons
 #pragma unroll
         for (int e = 0; e < NEQ; ++e) FxH[e * TY + i] = F[e];
         FxH[NEQ * TY + i] = uf;
+    }
+    __syncthreads();                                                // S2: y right states have been read, rim fluxes are visible
+    if constexpr (D >= 2) {
+#pragma unroll
+        for (int e = 0; e < NEQ; ++e) B.X[e * NT + tid] = Fy[e];
+        B.X8[tid] = ufy;
     }
     __syncthreads();                                                // S3: fluxes are visible
     if (i == 0) {
@@ -320,16 +330,15 @@ __global__ void __launch_bounds__(FTX *TY, 1)
     const int x0 = bx * FTX, y0 = by * TY;
     const int k0 = bs * seg, k1 = min(k0 + seg, g.n[2]);
     const bool active = x0 + i < g.n[0] && y0 + j < g.n[1];
-    const long long col = (long long)(x0 + i + NG) + (long long)(y0 + j + NG) * g.sy;     // own cell within a plane
+    const int col = (x0 + i + NG) + (y0 + j + NG) * (int)g.sy;      // own cell within a plane (a plane fits an int)
     // own column as a SOURCE (a thread past the domain edge still computes on admissible data)
-    const long long scol = staged_source<2>(g, x0, y0, 0, i + NG, j + NG);
+    const int scol = (int)staged_source<2>(g, x0, y0, 0, i + NG, j + NG);
     double *const pcw = P + (j + NG) * FPX + (i + NG);
     const double cx = o.coef * g.inv_dx[0], cy = o.coef * g.inv_dx[1], cz = o.coef * g.inv_dx[2];
 
     // halo cells of this thread: staged position and in-plane source.  Halo positions are numbered in row-major
     // order of the staged plane, skipping the interior block.
-    int hpos[NHT];
-    long long hsrc[NHT];
+    int hpos[NHT], hsrc[NHT];
 #pragma unroll
     for (int t = 0; t < NHT; ++t) {
         const int h = tid + t * NT;
@@ -342,7 +351,7 @@ __global__ void __launch_bounds__(FTX *TY, 1)
         } else if (h < NH) c = (NG + TY) * FPX + (h - TOP - 2 * NG * TY);
         hpos[t] = c;
         const int jj = c / FPX, ii = c - jj * FPX;
-        hsrc[t] = staged_source<2>(g, x0, y0, 0, ii, jj);
+        hsrc[t] = (int)staged_source<2>(g, x0, y0, 0, ii, jj);
     }
     auto zoff = [&](int p) -> long long {
         return (long long)(bc_source(min(max(p, -NG), g.n[2] + NG - 1), g.n[2], g.bc_lo[2], g.bc_hi[2]) + NG) * g.sz;
@@ -372,83 +381,22 @@ __global__ void __launch_bounds__(FTX *TY, 1)
     };
 
     double Fmz[NEQ], ufmz = 0.0;                                    // flux and face velocity of the previous z face
+    double vprev[NEQ];                                              // own cell of the plane that just left the ring
 #pragma unroll
-    for (int e = 0; e < NEQ; ++e) Fmz[e] = 0.0;
+    for (int e = 0; e < NEQ; ++e) { Fmz[e] = 0.0; vprev[e] = 0.0; }
 
-    // Commit groups are issued in the order column, halo, base in every iteration (empty ones included) and each
-    // is consumed one iteration later in the same order, so the wait is always "all but the two youngest".
-    const int pstart = k0 - NG, pend = k1 + NG;
-    stage_column(pstart);
-    cp_async_commit();
-    cp_async_commit();
-    cp_async_commit();
-#pragma unroll 1
-    for (int m = pstart; m < pend; ++m) {
-        const int n = m - pstart;                                   // planes brought in before this one
-        const int ip = m - NG;                                      // plane differenced in x and y in this iteration
-        const bool inplane = ip >= k0;                              // block-uniform (ip < k1 always)
-
-        // ---- plane m of the own column: raw q (staged) -> primitives, in registers ----
-        cp_async_wait<2>();
-        double wn[NEQ];
-        {
-            double qc[NEQ];
+    // cons->prim of the staged raw values, in place and thread-private: own column of the next plane (SQ) and this
+    // thread's halo cells of the next staged plane (SH)
+    auto convert_staged = [&](bool column, bool halo) {
+        if (column) {
+            double qc[NEQ], wc[NEQ];
 #pragma unroll
             for (int e = 0; e < NEQ; ++e) qc[e] = SQ[e * NT + tid];
-            cons_to_prim_cell<D, NF>(qc, eos, wn);
+            cons_to_prim_cell<D, NF>(qc, eos, wc);
+#pragma unroll
+            for (int e = 0; e < NEQ; ++e) SQ[e * NT + tid] = wc[e];
         }
-        if (m + 1 < pend) stage_column(m + 1);
-        cp_async_commit();
-
-        // ---- z: reconstruct cell m - 2, solve face (m - 2) - 1/2, difference for cell m - 3 = ip ----
-        double acc[NEQ];
-#pragma unroll
-        for (int e = 0; e < NEQ; ++e) acc[e] = 0.0;
-        if (n >= 4) {
-            const int c = m - 2;
-            const double *const rb = R + ((m + 1) & 3) * NEQ * NT + tid;      // plane m - 3
-            const double *const rc = R + ((m + 2) & 3) * NEQ * NT + tid;      // plane m - 2
-            const double *const rd = R + ((m + 3) & 3) * NEQ * NT + tid;      // plane m - 1
-            double vLp[NEQ], vL[NEQ], vR[NEQ], ab[NA1];
-#pragma unroll
-            for (int e = 0; e < NEQ; ++e) vLp[e] = park[e * NT + tid];
-#pragma unroll
-            for (int e = 0; e < NEQ; ++e) {
-                const double va = pcw[e * PPL], vb = rb[e * NT], vc = rc[e * NT], vd = rd[e * NT];
-                weno5(vc, vb - va, vc - vb, vd - vc, wn[e] - vd, eos.weno_eps4, vL[e], vR[e]);
-                if (e >= I::A) ab[e - I::A] = vb;
-            }
-#pragma unroll
-            for (int e = 0; e < NEQ; ++e) park[e * NT + tid] = vL[e];
-            if (c >= k0) {
-                double Fp[NEQ], ufp;
-                hllc<D, NF, 2>(vLp, vR, eos, Fp, ufp);
-                const double du = ufp - ufmz;
-#pragma unroll
-                for (int e = 0; e < NEQ; ++e) {
-                    double rr = Fmz[e] - Fp[e];
-                    if (e >= I::A) rr = fma(ab[e - I::A], du, rr);
-                    acc[e] = cz * rr;                               // meaningful when c > k0, i.e. when ip >= k0
-                    Fmz[e] = Fp[e];
-                }
-                ufmz = ufp;
-            }
-        }
-        __syncthreads();                                            // B1: the previous iteration's reads of P and X are over
-
-        // ---- plane m enters the ring (slot of plane m - 4, which served as X); plane ip = m - 3 is staged ----
-        {
-            double *const rs = R + (m & 3) * NEQ * NT + tid;
-#pragma unroll
-            for (int e = 0; e < NEQ; ++e) rs[e * NT] = wn[e];
-        }
-        if (n >= 3) {
-            const double *const rp = R + ((m + 1) & 3) * NEQ * NT + tid;
-#pragma unroll
-            for (int e = 0; e < NEQ; ++e) pcw[e * PPL] = rp[e * NT];
-        }
-        cp_async_wait<2>();
-        if (inplane) {
+        if (halo) {
 #pragma unroll
             for (int t = 0; t < NHT; ++t) {
                 if (tid + t * NT < NH) {
@@ -457,33 +405,110 @@ __global__ void __launch_bounds__(FTX *TY, 1)
                     for (int e = 0; e < NEQ; ++e) qc[e] = SH[(e * NHT + t) * NT + tid];
                     cons_to_prim_cell<D, NF>(qc, eos, wc);
 #pragma unroll
-                    for (int e = 0; e < NEQ; ++e) P[e * PPL + hpos[t]] = wc[e];
+                    for (int e = 0; e < NEQ; ++e) SH[(e * NHT + t) * NT + tid] = wc[e];
                 }
             }
         }
-        if (ip + 1 >= k0 && ip + 1 < k1) stage_halo(ip + 1);
-        cp_async_commit();
-        double qnv[NEQ];                                            // q_n of the cell written below (prefetched into L2)
-        if (inplane && active) {
-            const long long cell = (long long)(ip + NG) * g.sz + col;
-            if (o.nbase > 1) {
+    };
+
+    // Iteration m: plane m enters the z window, plane ip = m - 3 is differenced in x and y and written.
+    //   top      wn <- SQ (primitives of plane m, converted during the previous iteration); issue raw column m + 1
+    //            z: cell m - 2 reconstructed, face (m - 2) - 1/2 solved, z part of cell ip; plane m -> ring
+    //   in-plane (three barriers) on P = plane ip; in its second block the raw column m + 1 and the raw halo of
+    //            plane ip + 1 are converted in place
+    //   bottom   out(ip) written; P restaged with plane ip + 1 (own cell from the ring, halo cells from SH);
+    //            raw q_s of cell ip + 1 and raw halo of plane ip + 2 issued
+    //   barrier  (P staged; the exchange buffer, which is the ring slot plane m + 1 goes to, is free)
+    const int pstart = k0 - NG, pend = k1 + NG;
+    stage_column(pstart);
+    cp_async_commit();
+    cp_async_wait<0>();
+    convert_staged(true, false);
+#pragma unroll 1
+    for (int m = pstart; m < pend; ++m) {
+        const int n = m - pstart;                                   // planes brought in before this one
+        const int ip = m - NG;
+        const bool inplane = ip >= k0;                              // block-uniform (ip < k1 always)
+        const bool next_inplane = ip + 1 >= k0 && ip + 1 < k1;
+
+        double wn[NEQ];
 #pragma unroll
-                for (int e = 0; e < NEQ; ++e) qnv[e] = o.qn[(long long)e * g.cells + cell];
+        for (int e = 0; e < NEQ; ++e) wn[e] = SQ[e * NT + tid];
+        if (m + 1 < pend) stage_column(m + 1);
+        cp_async_commit();
+        if (m + 2 < pend) {                                         // the column after that: into L2
+            const double *src = q + zoff(m + 2) + scol;
+#pragma unroll
+            for (int e = 0; e < NEQ; ++e) prefetch_l2(src + (long long)e * g.cells);
+        }
+
+        // ---- z: reconstruct cell m - 2, solve face (m - 2) - 1/2, difference for cell m - 3 = ip ----
+        double acc[NEQ];
+#pragma unroll
+        for (int e = 0; e < NEQ; ++e) acc[e] = 0.0;
+        if (n >= 3) {
+            const double *const rb = R + ((m + 1) & 3) * NEQ * NT + tid;      // plane m - 3
+            double vb[NEQ];
+#pragma unroll
+            for (int e = 0; e < NEQ; ++e) vb[e] = rb[e * NT];
+            if (n >= 4) {
+                const int c = m - 2;
+                const double *const rc = R + ((m + 2) & 3) * NEQ * NT + tid;  // plane m - 2
+                const double *const rd = R + ((m + 3) & 3) * NEQ * NT + tid;  // plane m - 1
+                double vLp[NEQ], vL[NEQ], vR[NEQ];
+#pragma unroll
+                for (int e = 0; e < NEQ; ++e) vLp[e] = park[e * NT + tid];
+#pragma unroll
+                for (int e = 0; e < NEQ; ++e) {
+                    const double vc = rc[e * NT], vd = rd[e * NT];
+                    weno5(vc, vb[e] - vprev[e], vc - vb[e], vd - vc, wn[e] - vd, eos.weno_eps4, vL[e], vR[e]);
+                }
+#pragma unroll
+                for (int e = 0; e < NEQ; ++e) park[e * NT + tid] = vL[e];
+                if (c >= k0) {
+                    double Fp[NEQ], ufp;
+                    hllc<D, NF, 2>(vLp, vR, eos, Fp, ufp);
+                    const double du = ufp - ufmz;
+#pragma unroll
+                    for (int e = 0; e < NEQ; ++e) {
+                        double rr = Fmz[e] - Fp[e];
+                        if (e >= I::A) rr = fma(vb[e], du, rr);
+                        acc[e] = cz * rr;                           // meaningful when c > k0, i.e. when ip >= k0
+                        Fmz[e] = Fp[e];
+                    }
+                    ufmz = ufp;
+                }
+            }
+#pragma unroll
+            for (int e = 0; e < NEQ; ++e) vprev[e] = vb[e];
+        }
+        {   // plane m enters the ring: the slot of plane m - 4 (the previous iteration's exchange buffer)
+            double *const rs = R + (m & 3) * NEQ * NT + tid;
+#pragma unroll
+            for (int e = 0; e < NEQ; ++e) rs[e * NT] = wn[e];
+        }
+
+        double qnv[NEQ];                                            // q_n of the cell written below (prefetched into L2)
+        const long long cell = (long long)(ip + NG) * g.sz + col;
+        auto early = [&]() {
+            if (active && o.nbase > 1) {
+#pragma unroll
+                for (int e = 0; e < NEQ; ++e) qnv[e] = __ldcg(o.qn + (long long)e * g.cells + cell);
                 if (ip + 1 < k1) {
 #pragma unroll
                     for (int e = 0; e < NEQ; ++e) prefetch_l2(o.qn + (long long)e * g.cells + cell + g.sz);
                 }
             }
-        }
-        __syncthreads();                                            // B2: plane ip is staged
-
+        };
+        auto mid = [&]() {                                          // q_s and the halo of plane ip + 1 have landed
+            cp_async_wait<1>();
+            convert_staged(false, next_inplane);
+        };
         if (inplane) {
             const InplaneBufs<D, NF, TY> B(P, rim, R + ((m + 1) & 3) * NEQ * NT, X8);
-            inplane_xy<D, NF, TY>(B, eos, cx, cy, acc);
+            inplane_xy<D, NF, TY>(B, eos, cx, cy, acc, early, mid);
             // ---- a5: out = ca q_n + cb q_s + coef L ----
-            cp_async_wait<2>();
             if (active) {
-                const long long cell = (long long)(ip + NG) * g.sz + col;
 #pragma unroll
                 for (int e = 0; e < NEQ; ++e) {
                     double v = acc[e];
@@ -492,9 +517,29 @@ __global__ void __launch_bounds__(FTX *TY, 1)
                     o.out[(long long)e * g.cells + cell] = v;
                 }
             }
+        } else {
+            mid();
         }
-        if (ip + 1 >= k0 && ip + 1 < k1) stage_base(ip + 1);
+
+        // ---- bottom: stage plane ip + 1 in P, issue the raw reads of the iteration after ----
+        if (next_inplane) {
+            const double *const rp = R + ((m + 2) & 3) * NEQ * NT + tid;      // plane m - 2 = ip + 1
+#pragma unroll
+            for (int e = 0; e < NEQ; ++e) pcw[e * PPL] = rp[e * NT];
+#pragma unroll
+            for (int t = 0; t < NHT; ++t) {
+                if (tid + t * NT < NH) {
+#pragma unroll
+                    for (int e = 0; e < NEQ; ++e) P[e * PPL + hpos[t]] = SH[(e * NHT + t) * NT + tid];
+                }
+            }
+            stage_base(ip + 1);
+        }
+        if (ip + 2 >= k0 && ip + 2 < k1) stage_halo(ip + 2);
+        cp_async_wait<0>();                                         // the raw column issued at the top has landed
         cp_async_commit();
+        convert_staged(m + 1 < pend, false);
+        __syncthreads();                                            // P is staged, the exchange buffer is free
     }
 }
 
