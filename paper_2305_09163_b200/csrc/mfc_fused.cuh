@@ -61,11 +61,11 @@ struct FusedCfg {
     static constexpr int nHy = D >= 2 ? 2 * NEQ * FTX : 0;
     static constexpr int nX8 = D >= 2 ? NT : 0;                     // face velocity row of the y exchange
     // 1D / 2D: the y exchange has its own buffer.  3D: it lives in the ring slot of the plane staged in P;
-    // ring (4 slots) + parked left state + staging of raw q: own column of plane m + 1, q_s of the cell being
-    // written, halo cells of plane m - 2
+    // ring (4 slots) + parked left state + staging of raw q: own column of the next plane, q_s of the cell being
+    // written, halo cells of the next two staged planes (double buffer)
     static constexpr int nX = D == 2 ? NEQ * NT : 0;
     static constexpr int nR = D == 3 ? 5 * NEQ * NT : 0;
-    static constexpr int nS = D == 3 ? NEQ * (2 * NT + NHT * NT) : 0;
+    static constexpr int nS = D == 3 ? NEQ * (2 * NT + 2 * NH) : 0;
     static constexpr int doubles = nP + nHx + nHy + nX8 + nX + nR + nS;
     static constexpr int bytes = doubles * (int)sizeof(double);
     static_assert(TY <= 16, "the x rim jobs are laid out for at most 16 rows");
@@ -320,7 +320,7 @@ __global__ void __launch_bounds__(FTX *TY, 1)
     double *const park = R + 4 * NEQ * NT;                          // [NEQ][NT]    left state of the next z face
     double *const SQ = park + NEQ * NT;                             // [NEQ][NT]    raw q, own column, next plane
     double *const SS = SQ + NEQ * NT;                               // [NEQ][NT]    raw q_s of the cell being written
-    double *const SH = SS + NEQ * NT;                               // [NEQ][NHT*NT] raw q, halo cells of the next staged plane
+    double *const SH = SS + NEQ * NT;                               // [2][NEQ][NH] raw q, halo cells of the next two staged planes
 
     const int tid = threadIdx.x, i = tid & 31, j = tid >> 5;
     int b = blockIdx.x;
@@ -330,15 +330,13 @@ __global__ void __launch_bounds__(FTX *TY, 1)
     const int x0 = bx * FTX, y0 = by * TY;
     const int k0 = bs * seg, k1 = min(k0 + seg, g.n[2]);
     const bool active = x0 + i < g.n[0] && y0 + j < g.n[1];
-    const int col = (x0 + i + NG) + (y0 + j + NG) * (int)g.sy;      // own cell within a plane (a plane fits an int)
     // own column as a SOURCE (a thread past the domain edge still computes on admissible data)
-    const int scol = (int)staged_source<2>(g, x0, y0, 0, i + NG, j + NG);
+    const int scol = (int)staged_source<2>(g, x0, y0, 0, i + NG, j + NG);   // == the own cell for an active thread
+    const int col = scol;
     double *const pcw = P + (j + NG) * FPX + (i + NG);
-    const double cx = o.coef * g.inv_dx[0], cy = o.coef * g.inv_dx[1], cz = o.coef * g.inv_dx[2];
-
     // halo cells of this thread: staged position and in-plane source.  Halo positions are numbered in row-major
     // order of the staged plane, skipping the interior block.
-    int hpos[NHT], hsrc[NHT];
+    int hpos[NHT];
 #pragma unroll
     for (int t = 0; t < NHT; ++t) {
         const int h = tid + t * NT;
@@ -350,8 +348,6 @@ __global__ void __launch_bounds__(FTX *TY, 1)
             c = (NG + r) * FPX + (k < NG ? k : FTX + k);
         } else if (h < NH) c = (NG + TY) * FPX + (h - TOP - 2 * NG * TY);
         hpos[t] = c;
-        const int jj = c / FPX, ii = c - jj * FPX;
-        hsrc[t] = (int)staged_source<2>(g, x0, y0, 0, ii, jj);
     }
     auto zoff = [&](int p) -> long long {
         return (long long)(bc_source(min(max(p, -NG), g.n[2] + NG - 1), g.n[2], g.bc_lo[2], g.bc_hi[2]) + NG) * g.sz;
@@ -361,14 +357,16 @@ __global__ void __launch_bounds__(FTX *TY, 1)
 #pragma unroll
         for (int e = 0; e < NEQ; ++e) cp_async8(SQ + e * NT + tid, src + (long long)e * g.cells);
     };
-    auto stage_halo = [&](int p) {                                  // raw q of plane p, this thread's halo cells -> SH
+    auto stage_halo = [&](int p) {                                  // raw q of plane p, this thread's halo cells -> SH[p & 1]
         const long long zo = zoff(p);
+        double *const sh = SH + (p & 1) * NEQ * NH;
 #pragma unroll
         for (int t = 0; t < NHT; ++t) {
             if (tid + t * NT < NH) {
-                const double *src = q + zo + hsrc[t];
+                const int jj = hpos[t] / FPX, ii = hpos[t] - jj * FPX;
+                const double *src = q + zo + staged_source<2>(g, x0, y0, 0, ii, jj);
 #pragma unroll
-                for (int e = 0; e < NEQ; ++e) cp_async8(SH + (e * NHT + t) * NT + tid, src + (long long)e * g.cells);
+                for (int e = 0; e < NEQ; ++e) cp_async8(sh + e * NH + t * NT + tid, src + (long long)e * g.cells);
             }
         }
     };
@@ -387,7 +385,7 @@ __global__ void __launch_bounds__(FTX *TY, 1)
 
     // cons->prim of the staged raw values, in place and thread-private: own column of the next plane (SQ) and this
     // thread's halo cells of the next staged plane (SH)
-    auto convert_staged = [&](bool column, bool halo) {
+    auto convert_staged = [&](bool column, int hplane) {            // hplane < 0: no halo to convert
         if (column) {
             double qc[NEQ], wc[NEQ];
 #pragma unroll
@@ -396,61 +394,88 @@ __global__ void __launch_bounds__(FTX *TY, 1)
 #pragma unroll
             for (int e = 0; e < NEQ; ++e) SQ[e * NT + tid] = wc[e];
         }
-        if (halo) {
+        if (hplane >= 0) {
+            double *const sh = SH + (hplane & 1) * NEQ * NH;
 #pragma unroll
             for (int t = 0; t < NHT; ++t) {
                 if (tid + t * NT < NH) {
                     double qc[NEQ], wc[NEQ];
 #pragma unroll
-                    for (int e = 0; e < NEQ; ++e) qc[e] = SH[(e * NHT + t) * NT + tid];
+                    for (int e = 0; e < NEQ; ++e) qc[e] = sh[e * NH + t * NT + tid];
                     cons_to_prim_cell<D, NF>(qc, eos, wc);
 #pragma unroll
-                    for (int e = 0; e < NEQ; ++e) SH[(e * NHT + t) * NT + tid] = wc[e];
+                    for (int e = 0; e < NEQ; ++e) sh[e * NH + t * NT + tid] = wc[e];
                 }
             }
         }
     };
 
-    // Iteration m: plane m enters the z window, plane ip = m - 3 is differenced in x and y and written.
-    //   top      wn <- SQ (primitives of plane m, converted during the previous iteration); issue raw column m + 1
-    //            z: cell m - 2 reconstructed, face (m - 2) - 1/2 solved, z part of cell ip; plane m -> ring
-    //   in-plane (three barriers) on P = plane ip; in its second block the raw column m + 1 and the raw halo of
-    //            plane ip + 1 are converted in place
-    //   bottom   out(ip) written; P restaged with plane ip + 1 (own cell from the ring, halo cells from SH);
-    //            raw q_s of cell ip + 1 and raw halo of plane ip + 2 issued
+    // Iteration m: plane ip = m - 3 (staged in P by the previous iteration) is differenced in x and y; then plane m
+    // enters the z window, cell m - 2 is reconstructed, face (m - 2) - 1/2 solved, and cell ip is complete.
+    //   in-plane (three barriers): q_n loads at its top; in its second block the raw column m (SQ) and the raw halo
+    //            of plane ip + 1 (SH) are converted to primitives in place
+    //   bottom   z part from wn = SQ; plane m -> ring; out(ip) written; P restaged with plane ip + 1 (own cell from
+    //            the ring, halo cells from SH); issue, as three commit groups in this order, {q_s of cell ip + 1},
+    //            {raw column m + 1}, {raw halo of plane m = ip + 3}
     //   barrier  (P staged; the exchange buffer, which is the ring slot plane m + 1 goes to, is free)
+    // The conversions need everything but the youngest group (the halo issued one iteration ago is used two
+    // iterations after its issue), so the only wait is "all but the youngest", half an iteration after the issue
+    // of q_s (L2-resident: it was this block's column three planes ago) and of the column.
     const int pstart = k0 - NG, pend = k1 + NG;
+    cp_async_commit();
     stage_column(pstart);
     cp_async_commit();
-    cp_async_wait<0>();
-    convert_staged(true, false);
+    cp_async_commit();
 #pragma unroll 1
     for (int m = pstart; m < pend; ++m) {
         const int n = m - pstart;                                   // planes brought in before this one
         const int ip = m - NG;
         const bool inplane = ip >= k0;                              // block-uniform (ip < k1 always)
         const bool next_inplane = ip + 1 >= k0 && ip + 1 < k1;
+        const long long cell = (long long)(ip + NG) * g.sz + col;
+        // the three coefficients are re-read from the constant bank every iteration rather than held in registers
+        double coef = o.coef;
+        asm volatile("" : "+d"(coef));
+        const double cx = coef * g.inv_dx[0], cy = coef * g.inv_dx[1], cz = coef * g.inv_dx[2];
 
+        double acc[NEQ], qnv[NEQ];                                  // qnv: q_n of the cell written below (prefetched into L2)
+#pragma unroll
+        for (int e = 0; e < NEQ; ++e) acc[e] = 0.0;
+        if (inplane) {
+            auto early = [&]() {
+                if (active && o.nbase > 1) {
+#pragma unroll
+                    for (int e = 0; e < NEQ; ++e) qnv[e] = __ldcg(o.qn + (long long)e * g.cells + cell);
+                    if (ip + 1 < k1) {
+#pragma unroll
+                        for (int e = 0; e < NEQ; ++e) prefetch_l2(o.qn + (long long)e * g.cells + cell + g.sz);
+                    }
+                }
+            };
+            auto mid = [&]() {                                      // q_s, column m and the halo of plane ip + 1 have landed
+                cp_async_wait<1>();
+                convert_staged(true, next_inplane ? ip + 1 : -1);
+            };
+            const InplaneBufs<D, NF, TY> B(P, rim, R + ((m + 1) & 3) * NEQ * NT, X8);
+            inplane_xy<D, NF, TY>(B, eos, cx, cy, acc, early, mid);
+        } else {
+            cp_async_wait<1>();
+            convert_staged(true, next_inplane ? ip + 1 : -1);
+        }
+
+        // ---- plane m of the own column (primitives since the conversion above) ----
         double wn[NEQ];
 #pragma unroll
         for (int e = 0; e < NEQ; ++e) wn[e] = SQ[e * NT + tid];
-        if (m + 1 < pend) stage_column(m + 1);
-        cp_async_commit();
-        if (m + 2 < pend) {                                         // the column after that: into L2
-            const double *src = q + zoff(m + 2) + scol;
-#pragma unroll
-            for (int e = 0; e < NEQ; ++e) prefetch_l2(src + (long long)e * g.cells);
-        }
 
         // ---- z: reconstruct cell m - 2, solve face (m - 2) - 1/2, difference for cell m - 3 = ip ----
-        double acc[NEQ];
-#pragma unroll
-        for (int e = 0; e < NEQ; ++e) acc[e] = 0.0;
         if (n >= 3) {
-            const double *const rb = R + ((m + 1) & 3) * NEQ * NT + tid;      // plane m - 3
+            // plane m - 3: in P when it has just been differenced in plane (its ring slot was the exchange buffer)
+            const double *const pb = inplane ? pcw : R + ((m + 1) & 3) * NEQ * NT + tid;
+            const int sb = inplane ? PPL : NT;
             double vb[NEQ];
 #pragma unroll
-            for (int e = 0; e < NEQ; ++e) vb[e] = rb[e * NT];
+            for (int e = 0; e < NEQ; ++e) vb[e] = pb[e * sb];
             if (n >= 4) {
                 const int c = m - 2;
                 const double *const rc = R + ((m + 2) & 3) * NEQ * NT + tid;  // plane m - 2
@@ -473,7 +498,7 @@ __global__ void __launch_bounds__(FTX *TY, 1)
                     for (int e = 0; e < NEQ; ++e) {
                         double rr = Fmz[e] - Fp[e];
                         if (e >= I::A) rr = fma(vb[e], du, rr);
-                        acc[e] = cz * rr;                           // meaningful when c > k0, i.e. when ip >= k0
+                        acc[e] = fma(cz, rr, acc[e]);               // meaningful when c > k0, i.e. when ip >= k0
                         Fmz[e] = Fp[e];
                     }
                     ufmz = ufp;
@@ -488,57 +513,42 @@ __global__ void __launch_bounds__(FTX *TY, 1)
             for (int e = 0; e < NEQ; ++e) rs[e * NT] = wn[e];
         }
 
-        double qnv[NEQ];                                            // q_n of the cell written below (prefetched into L2)
-        const long long cell = (long long)(ip + NG) * g.sz + col;
-        auto early = [&]() {
-            if (active && o.nbase > 1) {
+        // ---- a5: out = ca q_n + cb q_s + coef L ----
+        if (inplane && active) {
 #pragma unroll
-                for (int e = 0; e < NEQ; ++e) qnv[e] = __ldcg(o.qn + (long long)e * g.cells + cell);
-                if (ip + 1 < k1) {
-#pragma unroll
-                    for (int e = 0; e < NEQ; ++e) prefetch_l2(o.qn + (long long)e * g.cells + cell + g.sz);
-                }
+            for (int e = 0; e < NEQ; ++e) {
+                double v = acc[e];
+                if (o.nbase > 0) v = fma(o.cb, SS[e * NT + tid], v);
+                if (o.nbase > 1) v = fma(o.ca, qnv[e], v);
+                o.out[(long long)e * g.cells + cell] = v;
             }
-        };
-        auto mid = [&]() {                                          // q_s and the halo of plane ip + 1 have landed
-            cp_async_wait<1>();
-            convert_staged(false, next_inplane);
-        };
-        if (inplane) {
-            const InplaneBufs<D, NF, TY> B(P, rim, R + ((m + 1) & 3) * NEQ * NT, X8);
-            inplane_xy<D, NF, TY>(B, eos, cx, cy, acc, early, mid);
-            // ---- a5: out = ca q_n + cb q_s + coef L ----
-            if (active) {
-#pragma unroll
-                for (int e = 0; e < NEQ; ++e) {
-                    double v = acc[e];
-                    if (o.nbase > 0) v = fma(o.cb, SS[e * NT + tid], v);
-                    if (o.nbase > 1) v = fma(o.ca, qnv[e], v);
-                    o.out[(long long)e * g.cells + cell] = v;
-                }
-            }
-        } else {
-            mid();
         }
 
-        // ---- bottom: stage plane ip + 1 in P, issue the raw reads of the iteration after ----
+        // ---- stage plane ip + 1 in P, issue the raw reads of the next iterations ----
         if (next_inplane) {
             const double *const rp = R + ((m + 2) & 3) * NEQ * NT + tid;      // plane m - 2 = ip + 1
 #pragma unroll
             for (int e = 0; e < NEQ; ++e) pcw[e * PPL] = rp[e * NT];
+            const double *const sh = SH + ((ip + 1) & 1) * NEQ * NH;
 #pragma unroll
             for (int t = 0; t < NHT; ++t) {
                 if (tid + t * NT < NH) {
 #pragma unroll
-                    for (int e = 0; e < NEQ; ++e) P[e * PPL + hpos[t]] = SH[(e * NHT + t) * NT + tid];
+                    for (int e = 0; e < NEQ; ++e) P[e * PPL + hpos[t]] = sh[e * NH + t * NT + tid];
                 }
             }
             stage_base(ip + 1);
         }
-        if (ip + 2 >= k0 && ip + 2 < k1) stage_halo(ip + 2);
-        cp_async_wait<0>();                                         // the raw column issued at the top has landed
         cp_async_commit();
-        convert_staged(m + 1 < pend, false);
+        if (m + 1 < pend) stage_column(m + 1);
+        cp_async_commit();
+        if (m >= k0 && m < k1) stage_halo(m);                       // plane ip + 3: the buffer the copy above just freed
+        cp_async_commit();
+        if (m + 2 < pend) {                                         // the column after that: into L2
+            const double *src = q + zoff(m + 2) + scol;
+#pragma unroll
+            for (int e = 0; e < NEQ; ++e) prefetch_l2(src + (long long)e * g.cells);
+        }
         __syncthreads();                                            // P is staged, the exchange buffer is free
     }
 }
