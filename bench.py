@@ -40,6 +40,20 @@ def measured_peaks():
     return 6650.0, "fallback"
 
 
+def ncu_traffic(workload: str, kernel: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` on `workload`, from the committed ncu
+    capture (profiles/r01_dram_traffic.csv names the report and the command); None when no capture is recorded."""
+    path = os.path.join(ROOT, "profiles", "r01_dram_traffic.csv")
+    if not os.path.exists(path):
+        return None
+    import csv
+    with open(path) as f:
+        for row in csv.DictReader(f):
+            if row["workload"] == workload and row["kernel"] == kernel:
+                return float(row["dram_read_bytes"]) + float(row["dram_write_bytes"])
+    return None
+
+
 class ClockSampler:
     """SM clock, power and throttle reasons sampled through NVML every few ms WHILE the timed region runs
     (the quantities of the B200_PROFILING.md clocks line; a polling thread sees a 100 ms region, an
@@ -116,6 +130,24 @@ def rhs_algorithmic(prob):
     # compulsory bytes of an RK stage: q_s read once, result written once, q_n read in two of the three stages
     doubles = neq * (1 + 1 + 2.0 / 3.0)
     return flops, 8.0 * doubles
+
+
+def reduce_over_ranks(ms_total, e2e_ms, state_ok, dist, device):
+    """Replicas-only multi-GPU rule: the job takes as long as its slowest rank (max over ranks of the
+    device-timed region and of the end-to-end time) and is valid only if every rank's state is finite."""
+    if dist is None:
+        return ms_total, e2e_ms, state_ok
+    import torch
+    t = torch.tensor([ms_total, e2e_ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ok = torch.tensor([1.0 if state_ok else 0.0], device=device, dtype=torch.float64)
+    dist.all_reduce(ok, op=dist.ReduceOp.MIN)
+    return float(t[0]), float(t[1]), bool(ok.item() > 0.5)
+
+
+def whole_job_grind(ms_step, cells_per_rank, world, neq):
+    """ns per (cell x equation x RHS evaluation) of the whole job: every rank advances its own replica."""
+    return ms_step * 1e6 / (cells_per_rank * world * neq * RHS_PER_STEP)
 
 
 def run_ours(args):
@@ -198,18 +230,12 @@ def run_ours(args):
     torch.cuda.synchronize()
     e2e_ms = (time.perf_counter() - t0) * 1e3 / e2e_steps
 
-    if dist:
-        t = torch.tensor([ms_total, e2e_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total, e2e_ms = float(t[0]), float(t[1])
-        ok = torch.tensor([1.0 if state_ok else 0.0], device="cuda")
-        dist.all_reduce(ok, op=dist.ReduceOp.MIN)
-        state_ok = bool(ok.item() > 0.5)
+    ms_total, e2e_ms, state_ok = reduce_over_ranks(ms_total, e2e_ms, state_ok, dist, "cuda")
 
     if rank == 0:
         ms_step = ms_total / args.steps
         work = prob.cells * world * neq * RHS_PER_STEP
-        grind = ms_step * 1e6 / work
+        grind = whole_job_grind(ms_step, prob.cells, world, neq)
         hbm_peak, hbm_src = measured_peaks()
         fp64_tf, fp64_ms = B.mfc_probe_dfma(local)
         # dominant kernel: the fused right-hand side (one launch per RK stage)
@@ -220,14 +246,18 @@ def run_ours(args):
         ach_tf = flops_cell * prob.cells / t_avg / 1e12
         t_hbm = bytes_cell * prob.cells / (hbm_peak * 1e9)
         t_alu = flops_cell * prob.cells / (fp64_tf * 1e12)
+        traffic = ncu_traffic(args.workload if not args.n else "", dom)
         if t_hbm >= t_alu:
             roof = {"kernel": dom, "bound": "hbm", "achieved": ach_gbs, "peak": hbm_peak, "unit": "GB/s",
-                    "frac": ach_gbs / hbm_peak, "traffic": None, "peak_source": f"MEASURED_PEAKS.json ({hbm_src})"}
+                    "frac": ach_gbs / hbm_peak, "traffic": traffic, "peak_source": f"MEASURED_PEAKS.json ({hbm_src})"}
         else:
             roof = {"kernel": dom, "bound": "alu", "achieved": ach_tf, "peak": fp64_tf, "unit": "TFLOP/s",
-                    "frac": ach_tf / fp64_tf, "traffic": None, "peak_source": "mfc_probe_dfma, measured in this run"}
+                    "frac": ach_tf / fp64_tf, "traffic": traffic,
+                    "peak_source": "mfc_probe_dfma (register-resident DFMA chains), measured in this run; DESIGN.md 6.1"}
         roof.update({"algorithmic_flops_per_cell": flops_cell, "algorithmic_bytes_per_cell": bytes_cell,
                      "avg_launch_ms": prof[dom]["ms_avg"], "hbm_frac": ach_gbs / hbm_peak, "fp64_frac": ach_tf / fp64_tf,
+                     "hbm_peak_gbs": hbm_peak, "hbm_peak_source": f"MEASURED_PEAKS.json ({hbm_src})",
+                     "traffic_source": "profiles/r01_dram_traffic.csv (ncu --set full)" if traffic else None,
                      "fp64_peak_measured_tflops": fp64_tf, "fp64_peak_nominal_tflops": FP64_NOMINAL_TFLOPS,
                      "kernel_ms_sum_over_step_ms": sum(v["ms_total"] for v in prof.values()) / ms_total})
         out = {

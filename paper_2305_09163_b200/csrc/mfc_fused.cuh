@@ -438,18 +438,14 @@ __global__ void __launch_bounds__(FTX *TY, 1)
         asm volatile("" : "+d"(coef));
         const double cx = coef * g.inv_dx[0], cy = coef * g.inv_dx[1], cz = coef * g.inv_dx[2];
 
-        double acc[NEQ], qnv[NEQ];                                  // qnv: q_n of the cell written below (prefetched into L2)
+        double acc[NEQ];
 #pragma unroll
         for (int e = 0; e < NEQ; ++e) acc[e] = 0.0;
         if (inplane) {
-            auto early = [&]() {
-                if (active && o.nbase > 1) {
+            auto early = [&]() {                                    // q_n of the next plane: into L2
+                if (active && o.nbase > 1 && ip + 1 < k1) {
 #pragma unroll
-                    for (int e = 0; e < NEQ; ++e) qnv[e] = __ldcg(o.qn + (long long)e * g.cells + cell);
-                    if (ip + 1 < k1) {
-#pragma unroll
-                        for (int e = 0; e < NEQ; ++e) prefetch_l2(o.qn + (long long)e * g.cells + cell + g.sz);
-                    }
+                    for (int e = 0; e < NEQ; ++e) prefetch_l2(o.qn + (long long)e * g.cells + cell + g.sz);
                 }
             };
             auto mid = [&]() {                                      // q_s, column m and the halo of plane ip + 1 have landed
@@ -463,19 +459,58 @@ __global__ void __launch_bounds__(FTX *TY, 1)
             convert_staged(true, next_inplane ? ip + 1 : -1);
         }
 
-        // ---- plane m of the own column (primitives since the conversion above) ----
-        double wn[NEQ];
+        // ---- bottom of the iteration.  q_n (in L2 since the previous iteration) is loaded now and used at the very
+        // end; q_s joins the in-plane part at once ----
+        double qnv[NEQ];
+        if (inplane && active) {
+            if (o.nbase > 1) {
 #pragma unroll
-        for (int e = 0; e < NEQ; ++e) wn[e] = SQ[e * NT + tid];
-
-        // ---- z: reconstruct cell m - 2, solve face (m - 2) - 1/2, difference for cell m - 3 = ip ----
-        if (n >= 3) {
-            // plane m - 3: in P when it has just been differenced in plane (its ring slot was the exchange buffer)
+                for (int e = 0; e < NEQ; ++e) qnv[e] = __ldcg(o.qn + (long long)e * g.cells + cell);
+            }
+            if (o.nbase > 0) {
+#pragma unroll
+                for (int e = 0; e < NEQ; ++e) acc[e] = fma(o.cb, SS[e * NT + tid], acc[e]);
+            }
+        }
+        // plane m of the own column (primitives since the conversion above) and plane m - 3 = ip: the latter sits in P
+        // when it has just been differenced in plane (its ring slot was the exchange buffer)
+        double wn[NEQ], vb[NEQ];
+        {
             const double *const pb = inplane ? pcw : R + ((m + 1) & 3) * NEQ * NT + tid;
             const int sb = inplane ? PPL : NT;
-            double vb[NEQ];
 #pragma unroll
-            for (int e = 0; e < NEQ; ++e) vb[e] = pb[e * sb];
+            for (int e = 0; e < NEQ; ++e) { wn[e] = SQ[e * NT + tid]; vb[e] = n >= 3 ? pb[e * sb] : 0.0; }
+        }
+        // "glue": plane ip + 1 -> P, raw reads of the next iterations issued.  No FP64 work: half of the warps of every
+        // scheduler run it BEFORE the z part and half AFTER it, so that it overlaps the other half's arithmetic
+        auto glue = [&]() {
+            if (next_inplane) {
+                const double *const rp = R + ((m + 2) & 3) * NEQ * NT + tid;  // plane m - 2 = ip + 1
+#pragma unroll
+                for (int e = 0; e < NEQ; ++e) pcw[e * PPL] = rp[e * NT];
+                const double *const sh = SH + ((ip + 1) & 1) * NEQ * NH;
+#pragma unroll
+                for (int t = 0; t < NHT; ++t) {
+                    if (tid + t * NT < NH) {
+#pragma unroll
+                        for (int e = 0; e < NEQ; ++e) P[e * PPL + hpos[t]] = sh[e * NH + t * NT + tid];
+                    }
+                }
+                stage_base(ip + 1);
+            }
+            cp_async_commit();
+            if (m + 1 < pend) stage_column(m + 1);
+            cp_async_commit();
+            if (m >= k0 && m < k1) stage_halo(m);                   // plane ip + 3: the buffer the copy above just freed
+            cp_async_commit();
+            if (m + 2 < pend) {                                     // the column after that: into L2
+                const double *src = q + zoff(m + 2) + scol;
+#pragma unroll
+                for (int e = 0; e < NEQ; ++e) prefetch_l2(src + (long long)e * g.cells);
+            }
+        };
+        auto zpart = [&]() {
+            // ---- z: reconstruct cell m - 2, solve face (m - 2) - 1/2, difference for cell m - 3 = ip ----
             if (n >= 4) {
                 const int c = m - 2;
                 const double *const rc = R + ((m + 2) & 3) * NEQ * NT + tid;  // plane m - 2
@@ -506,48 +541,23 @@ __global__ void __launch_bounds__(FTX *TY, 1)
             }
 #pragma unroll
             for (int e = 0; e < NEQ; ++e) vprev[e] = vb[e];
-        }
-        {   // plane m enters the ring: the slot of plane m - 4 (the previous iteration's exchange buffer)
+            // plane m enters the ring: the slot of plane m - 4 (the previous iteration's exchange buffer)
             double *const rs = R + (m & 3) * NEQ * NT + tid;
 #pragma unroll
             for (int e = 0; e < NEQ; ++e) rs[e * NT] = wn[e];
-        }
-
-        // ---- a5: out = ca q_n + cb q_s + coef L ----
-        if (inplane && active) {
+            // ---- a5: out = ca q_n + cb q_s + coef L ----
+            if (inplane && active) {
 #pragma unroll
-            for (int e = 0; e < NEQ; ++e) {
-                double v = acc[e];
-                if (o.nbase > 0) v = fma(o.cb, SS[e * NT + tid], v);
-                if (o.nbase > 1) v = fma(o.ca, qnv[e], v);
-                o.out[(long long)e * g.cells + cell] = v;
+                for (int e = 0; e < NEQ; ++e)
+                    o.out[(long long)e * g.cells + cell] = o.nbase > 1 ? fma(o.ca, qnv[e], acc[e]) : acc[e];
             }
-        }
-
-        // ---- stage plane ip + 1 in P, issue the raw reads of the next iterations ----
-        if (next_inplane) {
-            const double *const rp = R + ((m + 2) & 3) * NEQ * NT + tid;      // plane m - 2 = ip + 1
-#pragma unroll
-            for (int e = 0; e < NEQ; ++e) pcw[e * PPL] = rp[e * NT];
-            const double *const sh = SH + ((ip + 1) & 1) * NEQ * NH;
-#pragma unroll
-            for (int t = 0; t < NHT; ++t) {
-                if (tid + t * NT < NH) {
-#pragma unroll
-                    for (int e = 0; e < NEQ; ++e) P[e * PPL + hpos[t]] = sh[e * NH + t * NT + tid];
-                }
-            }
-            stage_base(ip + 1);
-        }
-        cp_async_commit();
-        if (m + 1 < pend) stage_column(m + 1);
-        cp_async_commit();
-        if (m >= k0 && m < k1) stage_halo(m);                       // plane ip + 3: the buffer the copy above just freed
-        cp_async_commit();
-        if (m + 2 < pend) {                                         // the column after that: into L2
-            const double *src = q + zoff(m + 2) + scol;
-#pragma unroll
-            for (int e = 0; e < NEQ; ++e) prefetch_l2(src + (long long)e * g.cells);
+        };
+        if ((j >> 2) & 1) {
+            glue();
+            zpart();
+        } else {
+            zpart();
+            glue();
         }
         __syncthreads();                                            // P is staged, the exchange buffer is free
     }

@@ -6,6 +6,9 @@
 #ifndef MFC_D
 #error "define MFC_D (1, 2 or 3) before including mfc_inst.cuh"
 #endif
+#ifndef MFC_TY_2F
+#define MFC_TY_2F (NF <= 2 ? 12 : 8)
+#endif
 #define MFC_CAT2(a, b) a##b
 #define MFC_CAT(a, b) MFC_CAT2(a, b)
 
@@ -34,7 +37,7 @@ constexpr int fused_ty()
 {
     if (D == 1) return 1;
     if (D == 2) return 8;
-    return NF <= 2 ? 12 : 8;
+    return MFC_TY_2F;
 }
 
 // z segment of the march: blocks = tiles * nseg should fill whole waves of the multiprocessors (one block per
