@@ -8,28 +8,29 @@
 //
 // Decomposition (3D).  A block owns a tile of FTX x TY cells in (x, y) and MARCHES along z over a segment of
 // the domain; thread (i, j) = (lane, warp) owns the column (x0 + i, y0 + j).  The z direction runs three
-// planes ahead of the in-plane directions, so that when plane p is differenced in x and y both of its z faces
-// are already known and the cell is written once, complete:
-//   * iteration m brings in plane m of the thread's own column (raw q staged by cp.async one iteration
-//     earlier, converted to primitives in registers), reconstructs cell m - 2 in z from the thread-private
-//     window (plane m - 4 in P, planes m - 3 .. m - 1 in a 4-slot shared-memory ring, plane m in registers),
-//     solves face (m - 2) - 1/2 with the left state parked by the previous iteration and differences it
-//     against the previous flux (registers): the z part of cell m - 3;
-//   * plane m - 3 is then laid out with a halo of 3 cells in x and y (P): interior from the ring, halo cells
-//     from raw q staged by cp.async and converted here (ghost cells take the wrapped / clamped interior cell,
-//     PAPER.md:168); its ring slot becomes the exchange buffer of the y direction;
+// planes ahead of the in-plane directions, so that when plane ip is differenced in x and y both of its z faces
+// are known by the end of the iteration and the cell is written once, complete.  Iteration m, ip = m - 3:
+//   * plane ip sits in P with a halo of 3 cells in x and y, laid out by the previous iteration: own cells from
+//     the ring of primitive planes, halo cells from raw q staged by cp.async two iterations earlier (ghost
+//     cells take the wrapped / clamped interior cell);
 //   * x: each thread reconstructs its own cell from P; right states and fluxes move between neighbouring
-//     lanes by warp shuffles (tile width = warp width);  y: same, through shared memory (X);
-//   * the rim of the tile (left state of face -1/2 from cell -1, right state of the face past the last cell,
-//     in x and in y) is reconstructed by the first three warps; the rim faces themselves are solved by one
-//     warp once the first lane / row has published its state;
-//   * out = ca q_n + cb q_s + coef (L_x + L_y + L_z): q_s of the cell is staged by cp.async at the top of the
-//     iteration, q_n (L2-prefetched one iteration ahead) is loaded at the start of the in-plane work.
-// Every global read is therefore issued long before its first use, by the thread that uses it: no block
+//     lanes by warp shuffles (tile width = warp width);  y: same, through shared memory (X = the ring slot
+//     plane ip left);  the rim of the tile (states of the cells just outside it, in x and in y) is
+//     reconstructed by the first four warps, the rim faces are solved by two warps;
+//   * while that runs, the raw column of plane m and the raw halo of plane ip + 1 (both landed) are converted
+//     to primitives in place (thread-private);
+//   * z: cell m - 2 is reconstructed from the thread-private window (plane m - 4 in registers, m - 3 in P,
+//     m - 2 and m - 1 in the ring, m just converted), face (m - 2) - 1/2 solved with the left state parked by
+//     the previous iteration and differenced against the previous flux (registers): the z part of cell ip;
+//   * one store: out = ca q_n + cb q_s + coef (L_x + L_y + L_z); q_s staged by cp.async, q_n prefetched into L2;
+//   * "glue": P is restaged with plane ip + 1 and the raw reads of the next iterations are issued.  It has no
+//     FP64 work, so half of the warps of every scheduler run it before the z part and half after it.
+// Every global read is issued at least an iteration before its first use, by the thread that uses it: no block
 // barrier is involved in the staging, only cp.async.wait_group.
 // FP64 issue needs instruction-level parallelism rather than many warps on this part (one warp per scheduler
-// with four independent chains already reaches 92 % of the DFMA peak), so a block is 8 - 12 warps with up to
-// 168 - 255 registers each and the seven variables are reconstructed as independent chains.
+// with four independent chains already reaches 92 % of the DFMA peak; weno5 x 7 + hllc alone run at 96 % with
+// 8 - 16 warps per SM), so a block is 8 - 12 warps with up to 168 - 255 registers each.  What the kernel loses
+// against that figure is lost where all warps of a scheduler are in non-FP64 code at the same time.
 // 1D / 2D: one plane, no march: the same in-plane code on a directly loaded tile.
 #pragma once
 #include "mfc_math.cuh"
@@ -412,11 +413,11 @@ __global__ void __launch_bounds__(FTX *TY, 1)
 
     // Iteration m: plane ip = m - 3 (staged in P by the previous iteration) is differenced in x and y; then plane m
     // enters the z window, cell m - 2 is reconstructed, face (m - 2) - 1/2 solved, and cell ip is complete.
-    //   in-plane (three barriers): q_n loads at its top; in its second block the raw column m (SQ) and the raw halo
-    //            of plane ip + 1 (SH) are converted to primitives in place
-    //   bottom   z part from wn = SQ; plane m -> ring; out(ip) written; P restaged with plane ip + 1 (own cell from
-    //            the ring, halo cells from SH); issue, as three commit groups in this order, {q_s of cell ip + 1},
-    //            {raw column m + 1}, {raw halo of plane m = ip + 3}
+    //   in-plane (three barriers): q_n of the next plane prefetched at its top; in its second block the raw column m
+    //            (SQ) and the raw halo of plane ip + 1 (SH) are converted to primitives in place
+    //   bottom   z part from wn = SQ; plane m -> ring; out(ip) written  ||  glue: P restaged with plane ip + 1 (own
+    //            cell from the ring, halo cells from SH); issue, as three commit groups in this order, {q_s of cell
+    //            ip + 1}, {raw column m + 1}, {raw halo of plane m = ip + 3}   (order of the two halves per warp group)
     //   barrier  (P staged; the exchange buffer, which is the ring slot plane m + 1 goes to, is free)
     // The conversions need everything but the youngest group (the halo issued one iteration ago is used two
     // iterations after its issue), so the only wait is "all but the youngest", half an iteration after the issue
