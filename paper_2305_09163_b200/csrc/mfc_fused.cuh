@@ -116,26 +116,38 @@ __device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, cons
     double *const FyH = B.HyL;                                      // [NEQ+1][FTX] over HyL, HyR[0]
 
     early();
-    // ---- rim states, one job per thread of the first warps: [0,16) left state of x face -1/2 (from cell -1),
-    // [16,32) right state of the x face past the tile, [32,64) / [64,96) the same in y, [96,112) right state of
-    // x face -1/2 (from cell 0: recomputed here so that the rim face can be solved before lane 0 publishes it) ----
-    for (int job = tid; job < 112; job += NT) {
-        const bool inx = job < 32 || job >= 96;
+    // ---- rim states, one job per thread of the first four warps, one SIDE per warp (only that side of the
+    // reconstruction is evaluated): warp 0 left state of y face -1/2 (from row -1), warp 1 right state of the y face
+    // past the tile, warp 2 left state of x face -1/2 (from cell -1), warp 3 right states of the x face past the tile
+    // (lanes 0..15) and of x face -1/2 (lanes 16..31, from cell 0: recomputed here so that the rim face can be
+    // solved before lane 0 publishes it) ----
+    for (int job = tid; job < 128; job += NT) {
+        const bool inx = job >= 64;
         if (!inx && D < 2) continue;
+        const bool left = inx ? job < 96 : job < 32;                // which side of the cell the state is taken from
         const int r = inx ? (job & 15) : (job & 31);
-        const bool left = inx ? job < 16 : job < 64;                // which side of the cell the state is taken from
-        if (!inx || r < TY) {
+        const bool x0 = job >= 112;
+        if ((!inx || r < TY) && !(inx && left && (job & 31) >= 16)) {
             const int st = inx ? 1 : FPX;                           // stride along the normal direction
-            const int cc = job >= 96 ? 0 : (left ? -1 : (inx ? FTX : TY));   // centre cell along the normal direction
+            const int cc = x0 ? 0 : (left ? -1 : (inx ? FTX : TY)); // centre cell along the normal direction
             const double *pb = inx ? P + (r + HY) * FPX + NG + cc : P + (HY + cc) * FPX + NG + r;
-            double *dst = inx ? (job >= 96 ? B.ExR : (left ? B.HxL : B.HxR)) + r : (left ? B.HyL : B.HyR) + r;
+            double *dst = inx ? (x0 ? B.ExR : (left ? B.HxL : B.HxR)) + r : (left ? B.HyL : B.HyR) + r;
             const int ds = inx ? TY : FTX;
+            double v, unused;
+            if (left) {
 #pragma unroll
-            for (int e = 0; e < NEQ; ++e) {
-                const double *s5 = pb + e * PPL;
-                double vl, vr;
-                weno5(s5[0], s5[-st] - s5[-2 * st], s5[0] - s5[-st], s5[st] - s5[0], s5[2 * st] - s5[st], eos.weno_eps4, vl, vr);
-                dst[e * ds] = left ? vl : vr;
+                for (int e = 0; e < NEQ; ++e) {
+                    const double *s5 = pb + e * PPL;
+                    weno5(s5[0], s5[-st] - s5[-2 * st], s5[0] - s5[-st], s5[st] - s5[0], s5[2 * st] - s5[st], eos.weno_eps4, v, unused);
+                    dst[e * ds] = v;
+                }
+            } else {
+#pragma unroll
+                for (int e = 0; e < NEQ; ++e) {
+                    const double *s5 = pb + e * PPL;
+                    weno5(s5[0], s5[-st] - s5[-2 * st], s5[0] - s5[-st], s5[st] - s5[0], s5[2 * st] - s5[st], eos.weno_eps4, unused, v);
+                    dst[e * ds] = v;
+                }
             }
         }
     }
@@ -335,8 +347,8 @@ __global__ void __launch_bounds__(FTX *TY, 1)
     const int scol = (int)staged_source<2>(g, x0, y0, 0, i + NG, j + NG);   // == the own cell for an active thread
     const int col = scol;
     double *const pcw = P + (j + NG) * FPX + (i + NG);
-    // halo cells of this thread: staged position and in-plane source.  Halo positions are numbered in row-major
-    // order of the staged plane, skipping the interior block.
+    // halo cells of this thread: staged position.  Halo positions are numbered in row-major order of the staged
+    // plane, skipping the interior block.
     int hpos[NHT];
 #pragma unroll
     for (int t = 0; t < NHT; ++t) {
