@@ -173,6 +173,9 @@ def run_ours(args):
     B.lib()
 
     prob, q = get_workload(args.workload, args.n)
+    if args.kapila:
+        import dataclasses
+        prob = dataclasses.replace(prob, name=prob.name + "+kapila", kapila=True)
     ctx = B.init_from_problem(prob, device=local, march_segment=args.segment)
     neq, ng, padded, elems = B.mfc_layout(ctx)
     stream = torch.cuda.current_stream().cuda_stream
@@ -344,6 +347,7 @@ def main():
     ap.add_argument("--cpu-n", type=int, default=128, help="cells per dimension of the cpu_baseline sample")
     ap.add_argument("--ref-n", type=int, default=96, help="cells per dimension of the --impl reference sample")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--kapila", action="store_true", help="switch the K div(u) source of PAPER.md Eq. 2 on (not the headline config)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -41,7 +41,7 @@ extern "C" {
 typedef enum {
     MFC_OK = 0,
     MFC_EINVAL = -1,       /* null pointer, bad shape, n_d < 3 in an active dimension, gamma <= 1, bad BC kind */
-    MFC_EUNSUPPORTED = -2, /* (ndim, n_fluids) outside the compiled template set */
+    MFC_EUNSUPPORTED = -2, /* (ndim, n_fluids) outside the compiled template set; kapila with n_fluids != 2 */
     MFC_ECUDA = -3,        /* CUDA runtime error (sticky); no device */
     MFC_ENOMEM = -4        /* device or host allocation failed */
 } mfc_status;
@@ -70,6 +70,9 @@ typedef struct {
     double cfl;        /* CFL number used by mfc_cfl_dt; <= 0 selects 0.3 */
     int device;        /* CUDA device ordinal; < 0 selects the current device */
     int march_segment; /* planes each block of the fused kernel marches along z (3D); <= 0 selects a heuristic */
+    int kapila;        /* != 0: Kapila model, the alpha row carries the source K div(u) with the two-fluid K of Eq. 2
+                          (PAPER.md:52, 60-62), cell-centred, on the same face-velocity differences as alpha div(u);
+                          needs n_fluids == 2 and volume fractions inside (0, 1).  0: Allaire model, K = 0 */
 } mfc_opts;
 
 typedef struct mfc_ctx mfc_ctx;
@@ -85,10 +88,10 @@ void mfc_destroy(mfc_ctx *ctx);
  * Any out pointer may be NULL. */
 int mfc_layout(const mfc_ctx *ctx, int *neq, int *ng, long long padded_n[3], long long *elems);
 
-/* L(q): one evaluation of the spatial operator, PAPER.md:105-130 (Eq. 6-10) with s(q) = 0, K = 0:
+/* L(q): one evaluation of the spatial operator, PAPER.md:105-130 (Eq. 6-10) with s(q) = 0 (K = 0 unless opts.kapila):
  *   cons->prim with ghost fill -> per direction WENO5-JS (Eq. 12,
  *   Listing 1) -> HLLC flux and face velocity (Eq. 13-14) ->
- *   rhs_k = sum_d (F_{k,-1/2} - F_{k,+1/2})/dx_d  [+ alpha_i sum_d (u_{+1/2} - u_{-1/2})/dx_d on alpha rows].
+ *   rhs_k = sum_d (F_{k,-1/2} - F_{k,+1/2})/dx_d  [+ (alpha_i + K) sum_d (u_{+1/2} - u_{-1/2})/dx_d on alpha rows].
  * q_dev is read (interior only); the interior of rhs_dev is written.  q_dev and rhs_dev must not alias. */
 int mfc_rhs(mfc_ctx *ctx, const double *q_dev, double *rhs_dev, void *stream);
 

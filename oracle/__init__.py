@@ -32,6 +32,7 @@ class _Problem(C.Structure):
         ("bc_lo", C.c_int * 3),
         ("bc_hi", C.c_int * 3),
         ("weno_eps", C.c_double),
+        ("kapila", C.c_int),
     ]
 
 
@@ -67,6 +68,7 @@ def lib():
         L.orc_rhs.argtypes = [pp, dp, dp]; L.orc_rhs.restype = None
         L.orc_rk3_step.argtypes = [pp, dp, C.c_double]; L.orc_rk3_step.restype = None
         L.orc_cfl_dt.argtypes = [pp, dp, C.c_double]; L.orc_cfl_dt.restype = C.c_double
+        L.orc_kapila_K.argtypes = [pp, C.c_double, C.c_double]; L.orc_kapila_K.restype = C.c_double
         L.orc_threads.argtypes = []; L.orc_threads.restype = C.c_int
         L.orc_set_threads.argtypes = [C.c_int]; L.orc_set_threads.restype = None
         _lib = L
@@ -96,11 +98,17 @@ class Oracle:
             P.gamma[i] = float(g)
             P.pi_inf[i] = float(pinf)
         P.weno_eps = float(prob.weno_eps)
+        P.kapila = 1 if getattr(prob, "kapila", False) else 0
+        assert not P.kapila or P.nf == 2, "the Kapila coefficient of Eq. 2 is the two-fluid one"
         self.P = P
         self.neq = self.L.orc_neq(C.byref(P))
         self.elems = self.L.orc_elems(C.byref(P))
         self.ndim = P.ndim
         self.nf = P.nf
+
+    def kapila_K(self, alpha1: float, p: float) -> float:
+        """K of PAPER.md Eq. 2 at one state (two fluids)."""
+        return float(self.L.orc_kapila_K(C.byref(self.P), float(alpha1), float(p)))
 
     # -- whole-array operations (q is [neq, pz, py, px], modified in place where noted) --
     def fill_ghosts(self, q: np.ndarray) -> None:

@@ -2,7 +2,8 @@
  * mfc_oracle.c  --  TEST INFRASTRUCTURE, NOT THE PRODUCT.
  *
  * Plain, slow, fp64 CPU statement of what the hot path computes: the right-hand side of the
- * 5-equation (Allaire, K = 0) diffuse-interface model with stiffened-gas EOS on a uniform grid,
+ * 5-equation diffuse-interface model (Allaire, K = 0; optionally the Kapila source K div(u) of Eq. 2, two
+ * fluids) with stiffened-gas EOS on a uniform grid,
  * driven by 3-stage TVD Runge-Kutta, exactly in the paper's order:
  *   ghost fill -> cons->prim -> per-direction WENO5-JS -> HLLC (+ face velocity) -> flux difference
  *   + alpha*div(u) -> RK stage combine;  plus the CFL time step.
@@ -43,6 +44,7 @@ typedef struct {
     double pi_inf[ORC_MAXF];
     int bc_lo[3], bc_hi[3]; /* 0 periodic, 1 extrapolation */
     double weno_eps;
+    int kapila;            /* 0: Allaire model (K = 0); 1: Kapila source K div(u) on the alpha row, two fluids (Eq. 2) */
 } orc_problem;
 
 static int neq_of(const orc_problem *P) { return 2 * P->nf + P->ndim; }
@@ -235,8 +237,24 @@ void orc_hllc(const orc_problem *P, int dir, const double *wL, const double *wR,
 }
 
 /* ------------------------------------------------------------------------------------------------
- * A7. RHS, PAPER.md:105-130 (Eq. 6-10) with s(q) = 0 and h = -alpha on the alpha rows (K = 0):
- *   L_k = sum_d (F^d_{k,-1/2} - F^d_{k,+1/2})/dx_d  [+ alpha_i * sum_d (u^d_{+1/2} - u^d_{-1/2})/dx_d]
+ * A6b. Kapila coefficient, PAPER.md:60-62 (Eq. 2), two fluids:
+ *   K = (rho_2 c_2^2 - rho_1 c_1^2) / (rho_2 c_2^2 / alpha_2 + rho_1 c_1^2 / alpha_1)
+ * (the denominator of Eq. 2 prints "rho_1 c_2^2": read as rho_1 c_1^2, reading B3).  For a stiffened
+ * gas (Eq. 1) c_i^2 = gamma_i (p + pi_inf_i) / rho_i, so rho_i c_i^2 = gamma_i (p + pi_inf_i).
+ * ---------------------------------------------------------------------------------------------- */
+double orc_kapila_K(const orc_problem *P, double alpha1, double p)
+{
+    const double alpha2 = 1.0 - alpha1;
+    const double rc1 = P->gamma[0] * (p + P->pi_inf[0]);
+    const double rc2 = P->gamma[1] * (p + P->pi_inf[1]);
+    return (rc2 - rc1) / (rc2 / alpha2 + rc1 / alpha1);
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * A7. RHS, PAPER.md:105-130 (Eq. 6-10) with s(q) = 0 and h = -alpha on the alpha rows:
+ *   L_k = sum_d (F^d_{k,-1/2} - F^d_{k,+1/2})/dx_d  [+ (alpha_i + K) * sum_d (u^d_{+1/2} - u^d_{-1/2})/dx_d]
+ * K = 0 (Allaire) unless P->kapila: then the cell-centred K of Eq. 2 multiplies the same
+ * face-velocity differences ("K div u").
  * Fills the ghosts of q, converts to primitives, then direction by direction: WENO on every line,
  * HLLC on every face, flux differences.  L has q's padded layout; only its interior is written.
  * ---------------------------------------------------------------------------------------------- */
@@ -290,8 +308,11 @@ void orc_rhs(const orc_problem *P, double *q, double *L)
                 cell = at(P, idx[0], idx[1], idx[2]);
                 for (int e = 0; e < neq; ++e)
                     L[(size_t)e * C + cell] += (Ff[(size_t)j * neq + e] - Ff[(size_t)(j + 1) * neq + e]) / P->dx[dir];
-                for (int i = 0; i < nf - 1; ++i)
-                    L[(size_t)(iA + i) * C + cell] += q[(size_t)(iA + i) * C + cell] * (uf[j + 1] - uf[j]) / P->dx[dir];
+                for (int i = 0; i < nf - 1; ++i) {
+                    double h = q[(size_t)(iA + i) * C + cell];
+                    if (P->kapila && nf == 2) h += orc_kapila_K(P, w[(size_t)iA * C + cell], w[(size_t)(nf + D) * C + cell]);
+                    L[(size_t)(iA + i) * C + cell] += h * (uf[j + 1] - uf[j]) / P->dx[dir];
+                }
             }
             free(vL); free(vR); free(Ff); free(uf);
         }

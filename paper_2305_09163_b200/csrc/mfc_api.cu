@@ -247,6 +247,7 @@ int mfc_init(mfc_ctx **out, const mfc_grid *grid, int n_fluids, const mfc_fluid 
     *out = nullptr;
     if (grid->ndim < 1 || grid->ndim > 3 || n_fluids < 1) return MFC_EINVAL;
     if (n_fluids > MFC_MAX_FLUIDS) return MFC_EUNSUPPORTED;
+    if (opts && opts->kapila && n_fluids != 2) return MFC_EUNSUPPORTED;
     for (int d = 0; d < grid->ndim; ++d) {
         if (grid->n[d] < MFC_NG || !(grid->hi[d] > grid->lo[d])) return MFC_EINVAL;
         if (bc->lo[d] != MFC_BC_PERIODIC && bc->lo[d] != MFC_BC_EXTRAP) return MFC_EINVAL;
@@ -304,6 +305,7 @@ int mfc_init(mfc_ctx **out, const mfc_grid *grid, int n_fluids, const mfc_fluid 
         e.dP[i] = Pm[i] - e.P_last;
     }
     e.weno_eps4 = 4.0 * eps;
+    e.kapila = (opts && opts->kapila) ? 1 : 0;
 
     c->segment = (opts && opts->march_segment > 0) ? opts->march_segment : 0;   // 0: the launcher's heuristic
 

@@ -192,7 +192,7 @@ __device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, cons
 #pragma unroll
         for (int e = 0; e < NEQ; ++e) {
             double rr = __shfl_up_sync(0xffffffffu, Fp[e], 1) - Fp[e];
-            if (e >= I::A) rr = fma(pc[e * PPL], du, rr);
+            if (e >= I::A) rr = fma(alpha_div_coef<NF>(eos, pc[e * PPL], pc[I::E * PPL]), du, rr);
             ax[e] = rr;                                             // lane 0 is redone below with the rim flux
         }
     }
@@ -235,7 +235,7 @@ __device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, cons
 #pragma unroll
         for (int e = 0; e < NEQ; ++e) {
             double rr = FxH[e * TY + j] - B.ExF[e * TY + j];
-            if (e >= I::A) rr = fma(pc[e * PPL], du, rr);
+            if (e >= I::A) rr = fma(alpha_div_coef<NF>(eos, pc[e * PPL], pc[I::E * PPL]), du, rr);
             ax[e] = rr;
         }
     }
@@ -248,7 +248,7 @@ __device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, cons
         for (int e = 0; e < NEQ; ++e) {
             const double fm = j == 0 ? FyH[e * FTX + i] : B.X[e * NT + tid - FTX];
             double rr = fm - Fy[e];
-            if (e >= I::A) rr = fma(pc[e * PPL], du, rr);
+            if (e >= I::A) rr = fma(alpha_div_coef<NF>(eos, pc[e * PPL], pc[I::E * PPL]), du, rr);
             acc[e] = fma(cy, rr, acc[e]);
         }
     }
@@ -545,7 +545,7 @@ __global__ void __launch_bounds__(FTX *TY, 1)
 #pragma unroll
                     for (int e = 0; e < NEQ; ++e) {
                         double rr = Fmz[e] - Fp[e];
-                        if (e >= I::A) rr = fma(vb[e], du, rr);
+                        if (e >= I::A) rr = fma(alpha_div_coef<NF>(eos, vb[e], vb[I::E]), du, rr);
                         acc[e] = fma(cz, rr, acc[e]);               // meaningful when c > k0, i.e. when ip >= k0
                         Fmz[e] = Fp[e];
                     }

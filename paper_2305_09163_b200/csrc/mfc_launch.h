@@ -30,6 +30,7 @@ struct Eos {
     // Gamma = G_last + sum_{i<nf-1} alpha_i dG_i ;  Pi likewise  (alpha_nf = 1 - sum alpha_i)
     double G_last, P_last, dG[MAX_NF], dP[MAX_NF];
     double weno_eps4;    // 4 * eps : smoothness indicators are carried scaled by 4
+    int kapila;          // 1: K div(u) source of PAPER.md Eq. 2 on the alpha row (two fluids); 0: Allaire, K = 0
 };
 
 // output stage of one evaluation of L (a4 + a5):

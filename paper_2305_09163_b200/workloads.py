@@ -52,6 +52,7 @@ class Problem:
     steps: int = 1
     seed: int | None = None
     notes: str = ""
+    kapila: bool = False  # K div(u) source of PAPER.md Eq. 2 on the alpha row (two fluids); False = Allaire
 
     @property
     def nf(self) -> int:

@@ -187,6 +187,21 @@ def test_uniform_state_has_exactly_zero_rhs_on_gpu(ndim, nf, periodic):
     assert np.all(got[it] == 0.0)
 
 
+# Kapila source: same parity bar with opts.kapila on
+@pytest.mark.parametrize("ndim", [1, 2, 3])
+@pytest.mark.parametrize("periodic", [True, False])
+def test_rhs_parity_kapila_source(ndim, periodic):
+    import dataclasses
+    prob, q = wl.random_state(ndim, SIZES[ndim], 2, seed=40 + ndim, periodic=periodic)
+    prob = dataclasses.replace(prob, kapila=True)
+    check_rhs(prob, q, march_segment=8)
+    # the source is really on: the alpha row differs from the Allaire one
+    with Gpu(prob) as g1, Gpu(dataclasses.replace(prob, kapila=False)) as g0:
+        it = prob.interior()
+        a1, a0 = g1.rhs(q)[it], g0.rhs(q)[it]
+    assert np.array_equal(a1[:-1], a0[:-1]) and not np.allclose(a1[-1], a0[-1], rtol=1e-6)
+
+
 def test_rhs_parity_cfg0():
     prob, q = wl.cfg0()
     check_rhs(prob, q)
@@ -287,6 +302,12 @@ def test_rk3_parity_random_states(ndim, nf):
     n = {1: (600,), 2: (130, 45), 3: (40, 29, 33)}[ndim]
     prob, q = wl.random_state(ndim, n, nf, seed=20 * ndim + nf, periodic=(nf != 2), rough=False)
     check_rk(prob, q, march_segment=8)
+
+
+def test_rk3_parity_kapila_source():
+    import dataclasses
+    prob, q = wl.random_state(3, (40, 29, 33), 2, seed=91, periodic=False, rough=False)
+    check_rk(dataclasses.replace(prob, kapila=True), q, march_segment=8)
 
 
 def test_rk3_parity_cfg0():

@@ -529,3 +529,60 @@ def test_cfl_takes_the_minimum_over_cells():
     q3[2, 0, NG + 4, NG + 4] = rho[0, 4, 4] * 1e6
     q3[4, 0, NG + 4, NG + 4] += 0.5 * rho[0, 4, 4] * 1e12
     assert orc.cfl_dt(q3, 1.0) < prob.dx[0] / 1e6
+
+
+# ---------------------------------------------------------------------------------------------
+# Kapila source K div(u) (Eq. 2; reading B3)
+# ---------------------------------------------------------------------------------------------
+def _kapila(prob):
+    import dataclasses
+    return dataclasses.replace(prob, kapila=True)
+
+
+def test_kapila_K_against_the_definition_with_per_fluid_sound_speeds():
+    """K from rho_i c_i^2 with c_i^2 = gamma_i (p + pi_i) / rho_i (stiffened gas, Eq. 1) at arbitrary phase densities;
+    antisymmetric under relabelling the fluids (alpha_2 = 1 - alpha_1 must evolve with -K); zero for equal fluids."""
+    prob, _ = wl.cfg0()
+    orc = oracle.Oracle(_kapila(prob))
+    (g1, pi1), (g2, pi2) = prob.fluids
+    rng = np.random.default_rng(3)
+    for _ in range(50):
+        a1, p = rng.uniform(1e-6, 1 - 1e-6), 10 ** rng.uniform(3, 9)
+        rho1, rho2 = rng.uniform(500, 1500), rng.uniform(0.1, 100)
+        c1sq, c2sq = g1 * (p + pi1) / rho1, g2 * (p + pi2) / rho2
+        K = (rho2 * c2sq - rho1 * c1sq) / (rho2 * c2sq / (1 - a1) + rho1 * c1sq / a1)
+        assert orc.kapila_K(a1, p) == pytest.approx(K, rel=1e-13)
+    import dataclasses
+    swapped = oracle.Oracle(dataclasses.replace(_kapila(prob), fluids=prob.fluids[::-1]))
+    assert swapped.kapila_K(0.7, 2.5e5) == pytest.approx(-orc.kapila_K(0.3, 2.5e5), rel=1e-13)
+    same = oracle.Oracle(dataclasses.replace(_kapila(prob), fluids=[prob.fluids[1], prob.fluids[1]]))
+    assert same.kapila_K(0.3, 1e5) == 0.0
+    # stiff liquid + gas: the gas takes all the compression, K -> -alpha_liquid
+    assert orc.kapila_K(0.3, 1e5) == pytest.approx(-0.3, rel=1e-3)
+    with pytest.raises(AssertionError):
+        oracle.Oracle(_kapila(wl.random_state(1, (8,), 3, seed=1)[0]))
+
+
+def test_kapila_source_on_a_uniform_compression_is_K_div_u():
+    """Uniform alpha, rho, p and u = -a (x - 1/2): WENO5 is exact for linear data, HLLC of equal states returns the
+    state, so alpha div(u) cancels the flux difference and the alpha row is exactly K du/dx = -a K."""
+    prob, _ = wl.random_state(1, (40,), 2, seed=1, periodic=False)
+    x = prob.centers(0)[None, None, :]
+    a_rate, a1, p = 300.0, 0.35, 2.0e5
+    one = np.ones_like(x)
+    q = wl.assemble(prob, [a1 * one, (1 - a1) * one], [1000 * one, 1.2 * one], [-a_rate * (x - 0.5)], p * one)
+    pk = _kapila(prob)
+    L0 = interior(prob, oracle.Oracle(prob).rhs(q.copy()))
+    L1 = interior(prob, oracle.Oracle(pk).rhs(q.copy()))
+    K = oracle.Oracle(pk).kapila_K(a1, p)
+    inner = slice(4, -4)                                          # away from the extrapolated ghost cells
+    assert np.max(np.abs(L0[-1][0, 0, inner])) <= 1e-9 * a_rate                       # Allaire: nothing
+    assert np.allclose(L1[-1][0, 0, inner], -a_rate * K, rtol=1e-10, atol=0)
+    assert np.array_equal(L0[:-1], L1[:-1])                       # every other row is untouched
+
+
+def test_kapila_changes_nothing_where_the_velocity_is_uniform():
+    prob, q = wl.cfg1(n=32)
+    L0 = interior(prob, oracle.Oracle(prob).rhs(q.copy()))
+    L1 = interior(prob, oracle.Oracle(_kapila(prob)).rhs(q.copy()))
+    assert np.allclose(L0[-1], L1[-1], rtol=0, atol=1e-9 * np.max(np.abs(L0[-1])))
