@@ -40,7 +40,7 @@ extern "C" {
 
 typedef enum {
     MFC_OK = 0,
-    MFC_EINVAL = -1,       /* null pointer, bad shape, n_d < 3 in an active dimension, gamma <= 1, bad BC kind */
+    MFC_EINVAL = -1,       /* null pointer, bad shape, n_d < 3 in an active dimension, gamma <= 1, bad BC kind or order */
     MFC_EUNSUPPORTED = -2, /* (ndim, n_fluids) outside the compiled template set; kapila with n_fluids != 2 */
     MFC_ECUDA = -3,        /* CUDA runtime error (sticky); no device */
     MFC_ENOMEM = -4        /* device or host allocation failed */
@@ -70,6 +70,8 @@ typedef struct {
     double cfl;        /* CFL number used by mfc_cfl_dt; <= 0 selects 0.3 */
     int device;        /* CUDA device ordinal; < 0 selects the current device */
     int march_segment; /* planes each block of the fused kernel marches along z (3D); <= 0 selects a heuristic */
+    int weno_order;    /* reconstruction: 5 = WENO5-JS (0 selects it), 3 = WENO3-JS, 1 = piecewise
+                          constant; the ghost width stays 3 whatever the order */
     int kapila;        /* != 0: Kapila model, the alpha row carries the source K div(u) with the two-fluid K of Eq. 2
                           (PAPER.md:52, 60-62), cell-centred, on the same face-velocity differences as alpha div(u);
                           needs n_fluids == 2 and volume fractions inside (0, 1).  0: Allaire model, K = 0 */

@@ -32,6 +32,7 @@ class _Problem(C.Structure):
         ("bc_lo", C.c_int * 3),
         ("bc_hi", C.c_int * 3),
         ("weno_eps", C.c_double),
+        ("weno_order", C.c_int),
         ("kapila", C.c_int),
     ]
 
@@ -68,6 +69,7 @@ def lib():
         L.orc_rhs.argtypes = [pp, dp, dp]; L.orc_rhs.restype = None
         L.orc_rk3_step.argtypes = [pp, dp, C.c_double]; L.orc_rk3_step.restype = None
         L.orc_cfl_dt.argtypes = [pp, dp, C.c_double]; L.orc_cfl_dt.restype = C.c_double
+        L.orc_weno3.argtypes = [C.c_double] * 4 + [dp, dp]; L.orc_weno3.restype = None
         L.orc_kapila_K.argtypes = [pp, C.c_double, C.c_double]; L.orc_kapila_K.restype = C.c_double
         L.orc_threads.argtypes = []; L.orc_threads.restype = C.c_int
         L.orc_set_threads.argtypes = [C.c_int]; L.orc_set_threads.restype = None
@@ -98,6 +100,8 @@ class Oracle:
             P.gamma[i] = float(g)
             P.pi_inf[i] = float(pinf)
         P.weno_eps = float(prob.weno_eps)
+        P.weno_order = int(getattr(prob, "weno_order", 5))
+        assert P.weno_order in (1, 3, 5)
         P.kapila = 1 if getattr(prob, "kapila", False) else 0
         assert not P.kapila or P.nf == 2, "the Kapila coefficient of Eq. 2 is the two-fluid one"
         self.P = P
@@ -165,6 +169,13 @@ def weno5(a, b, c, d, e, eps=1e-16):
     vL = C.c_double()
     vR = C.c_double()
     lib().orc_weno5(float(a), float(b), float(c), float(d), float(e), float(eps), C.byref(vL), C.byref(vR))
+    return vL.value, vR.value
+
+
+def weno3(b, c, d, eps=1e-16):
+    vL = C.c_double()
+    vR = C.c_double()
+    lib().orc_weno3(float(b), float(c), float(d), float(eps), C.byref(vL), C.byref(vR))
     return vL.value, vR.value
 
 

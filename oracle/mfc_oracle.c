@@ -44,6 +44,7 @@ typedef struct {
     double pi_inf[ORC_MAXF];
     int bc_lo[3], bc_hi[3]; /* 0 periodic, 1 extrapolation */
     double weno_eps;
+    int weno_order;        /* 5 (WENO5-JS), 3 (WENO3-JS) or 1 (piecewise constant) */
     int kapila;            /* 0: Allaire model (K = 0); 1: Kapila source K div(u) on the alpha row, two fluids (Eq. 2) */
 } orc_problem;
 
@@ -176,6 +177,38 @@ void orc_weno5(double a, double b, double c, double d, double e, double eps, dou
 }
 
 /* ------------------------------------------------------------------------------------------------
+ * A5b. Lower-order variants of the same reconstruction (Eq. 12 with k = 2, "the third-order
+ * variant", and k = 1).  WENO3-JS: two 2-cell candidates per side, ideal weights 1/3 (upwind-biased pair) and
+ * 2/3 (centred pair), beta_0 = (w_i - w_{i-1})^2, beta_1 = (w_{i+1} - w_i)^2, same alpha = d / (beta + eps)^2.
+ * ---------------------------------------------------------------------------------------------- */
+void orc_weno3(double b, double c, double d, double eps, double *vL, double *vR)
+{
+    const double b0 = (c - b) * (c - b), b1 = (d - c) * (d - c);
+    {   /* left state at i+1/2 */
+        const double p0 = -0.5 * b + 1.5 * c, p1 = 0.5 * c + 0.5 * d;
+        const double a0 = (1.0 / 3.0) / ((b0 + eps) * (b0 + eps));
+        const double a1 = (2.0 / 3.0) / ((b1 + eps) * (b1 + eps));
+        const double s = a0 + a1;
+        *vL = (a0 / s) * p0 + (a1 / s) * p1;
+    }
+    {   /* right state at i-1/2: mirror image (b <-> d) */
+        const double p0 = -0.5 * d + 1.5 * c, p1 = 0.5 * c + 0.5 * b;
+        const double a0 = (1.0 / 3.0) / ((b1 + eps) * (b1 + eps));
+        const double a1 = (2.0 / 3.0) / ((b0 + eps) * (b0 + eps));
+        const double s = a0 + a1;
+        *vR = (a0 / s) * p0 + (a1 / s) * p1;
+    }
+}
+
+/* the reconstruction of the order the problem asks for, on the stencil a..e = w_{i-2..i+2} */
+void orc_reconstruct(const orc_problem *P, double a, double b, double c, double d, double e, double *vL, double *vR)
+{
+    if (P->weno_order == 3) orc_weno3(b, c, d, P->weno_eps, vL, vR);
+    else if (P->weno_order == 1) { *vL = c; *vR = c; }
+    else orc_weno5(a, b, c, d, e, P->weno_eps, vL, vR);
+}
+
+/* ------------------------------------------------------------------------------------------------
  * A6. HLLC, PAPER.md:152-164 (Eq. 13-14), with the face velocity of PAPER.md:126-136 (Eq. 10 and the
  * garbled equation after section 3.2: the Riemann solver returns F and u; reading B5).
  *   s_L = min(u_L - c_L, u_R - c_R), s_R = max(u_L + c_L, u_R + c_R)                  (reading B11)
@@ -292,8 +325,8 @@ void orc_rhs(const orc_problem *P, double *q, double *L)
                         idx[dir] = ORC_NG + j + s;
                         st[s + 2] = w[(size_t)e * C + at(P, idx[0], idx[1], idx[2])];
                     }
-                    orc_weno5(st[0], st[1], st[2], st[3], st[4], P->weno_eps,
-                              &vL[(size_t)(j + 1) * neq + e], &vR[(size_t)(j + 1) * neq + e]);
+                    orc_reconstruct(P, st[0], st[1], st[2], st[3], st[4],
+                                    &vL[(size_t)(j + 1) * neq + e], &vR[(size_t)(j + 1) * neq + e]);
                 }
             }
             /* HLLC: faces f = j+1/2, j = -1..n-1; left state from cell j, right state from cell j+1
@@ -329,7 +362,7 @@ void orc_line(const orc_problem *P, int dir, int n, const double *w, double *vL,
     for (int j = -1; j <= n; ++j)
         for (int e = 0; e < neq; ++e) {
             const double *s = w + (size_t)e * np + ORC_NG + j;
-            orc_weno5(s[-2], s[-1], s[0], s[1], s[2], P->weno_eps, &vL[(size_t)e * (n + 2) + j + 1], &vR[(size_t)e * (n + 2) + j + 1]);
+            orc_reconstruct(P, s[-2], s[-1], s[0], s[1], s[2], &vL[(size_t)e * (n + 2) + j + 1], &vR[(size_t)e * (n + 2) + j + 1]);
         }
     for (int j = -1; j <= n - 1; ++j) {
         double wl[ORC_MAXEQ], wr[ORC_MAXEQ], f[ORC_MAXEQ];

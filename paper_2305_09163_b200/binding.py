@@ -51,7 +51,7 @@ class mfc_bc(C.Structure):
 
 class mfc_opts(C.Structure):
     _fields_ = [("weno_eps", C.c_double), ("cfl", C.c_double), ("device", C.c_int), ("march_segment", C.c_int),
-                ("kapila", C.c_int)]
+                ("weno_order", C.c_int), ("kapila", C.c_int)]
 
 
 _lib = None
@@ -104,7 +104,8 @@ def mfc_version() -> str:
     return lib().mfc_version().decode()
 
 
-def mfc_init(grid_n, lo, hi, fluids, bc_lo, bc_hi, *, weno_eps=1e-16, cfl=0.3, device=-1, march_segment=0, kapila=False):
+def mfc_init(grid_n, lo, hi, fluids, bc_lo, bc_hi, *, weno_eps=1e-16, cfl=0.3, device=-1, march_segment=0, weno_order=5,
+             kapila=False):
     """grid_n / lo / hi: one entry per active dimension; fluids: [(gamma, pi_inf), ...]; returns the context handle."""
     ndim = len(grid_n)
     g = mfc_grid()
@@ -119,7 +120,7 @@ def mfc_init(grid_n, lo, hi, fluids, bc_lo, bc_hi, *, weno_eps=1e-16, cfl=0.3, d
     fl = (mfc_fluid * max(1, len(fluids)))()
     for i, (gam, pinf) in enumerate(fluids):
         fl[i].gamma, fl[i].pi_inf = float(gam), float(pinf)
-    o = mfc_opts(float(weno_eps), float(cfl), int(device), int(march_segment), 1 if kapila else 0)
+    o = mfc_opts(float(weno_eps), float(cfl), int(device), int(march_segment), int(weno_order), 1 if kapila else 0)
     h = C.c_void_p()
     _check(lib().mfc_init(C.byref(h), C.byref(g), len(fluids), fl, C.byref(b), C.byref(o)), "mfc_init")
     return h
@@ -193,4 +194,5 @@ def init_from_problem(prob, **kw):
     """mfc_init from a workloads.Problem-like object (ndim, n, lo, hi, fluids, bc_lo, bc_hi, weno_eps, cfl)."""
     D = prob.ndim
     return mfc_init(prob.n[:D], prob.lo[:D], prob.hi[:D], prob.fluids, prob.bc_lo[:D], prob.bc_hi[:D],
-                    weno_eps=prob.weno_eps, cfl=prob.cfl, kapila=getattr(prob, "kapila", False), **kw)
+                    weno_eps=prob.weno_eps, cfl=prob.cfl, weno_order=getattr(prob, "weno_order", 5),
+                    kapila=getattr(prob, "kapila", False), **kw)

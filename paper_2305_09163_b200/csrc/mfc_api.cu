@@ -22,13 +22,13 @@ cudaError_t launch_prim(int ndim, int nf, const Geo &g, const Eos &e, const doub
     }
     return cudaErrorInvalidValue;
 }
-cudaError_t launch_rhs(int ndim, int nf, const Geo &g, const Eos &e, const double *q, const SweepOut &o, int segment,
+cudaError_t launch_rhs(int ndim, int nf, int order, const Geo &g, const Eos &e, const double *q, const SweepOut &o, int segment,
                        cudaStream_t s)
 {
     switch (ndim) {
-        case 1: return launch_rhs_d1(nf, g, e, q, o, segment, s);
-        case 2: return launch_rhs_d2(nf, g, e, q, o, segment, s);
-        case 3: return launch_rhs_d3(nf, g, e, q, o, segment, s);
+        case 1: return launch_rhs_d1(nf, order, g, e, q, o, segment, s);
+        case 2: return launch_rhs_d2(nf, order, g, e, q, o, segment, s);
+        case 3: return launch_rhs_d3(nf, order, g, e, q, o, segment, s);
     }
     return cudaErrorInvalidValue;
 }
@@ -42,13 +42,13 @@ cudaError_t launch_cfl(int ndim, int nf, const Geo &g, const Eos &e, const doubl
     }
     return cudaErrorInvalidValue;
 }
-cudaError_t launch_line(int ndim, int nf, int dir, const Eos &e, int n, const double *w, double *vL, double *vR,
+cudaError_t launch_line(int ndim, int nf, int order, int dir, const Eos &e, int n, const double *w, double *vL, double *vR,
                         double *F, double *uf, cudaStream_t s)
 {
     switch (ndim) {
-        case 1: return launch_line_d1(nf, dir, e, n, w, vL, vR, F, uf, s);
-        case 2: return launch_line_d2(nf, dir, e, n, w, vL, vR, F, uf, s);
-        case 3: return launch_line_d3(nf, dir, e, n, w, vL, vR, F, uf, s);
+        case 1: return launch_line_d1(nf, order, dir, e, n, w, vL, vR, F, uf, s);
+        case 2: return launch_line_d2(nf, order, dir, e, n, w, vL, vR, F, uf, s);
+        case 3: return launch_line_d3(nf, order, dir, e, n, w, vL, vR, F, uf, s);
     }
     return cudaErrorInvalidValue;
 }
@@ -84,7 +84,7 @@ struct EventPair {
 }  // namespace mfc
 
 struct mfc_ctx {
-    int ndim = 0, nf = 0, neq = 0, device = 0, segment = 0;
+    int ndim = 0, nf = 0, neq = 0, device = 0, segment = 0, order = 5;
     double cfl = 0.3;
     long long elems = 0;
     mfc::Geo g{};
@@ -169,7 +169,7 @@ int eval_L(mfc_ctx *c, const double *q_in, const SweepOut &o, cudaStream_t s)
     cudaError_t err;
     {
         Timed t(c, MFC_K_RHS, s);
-        err = launch_rhs(c->ndim, c->nf, c->g, c->e, q_in, o, c->segment, s);
+        err = launch_rhs(c->ndim, c->nf, c->order, c->g, c->e, q_in, o, c->segment, s);
     }
     return cuda_to_status(err);
 }
@@ -248,6 +248,8 @@ int mfc_init(mfc_ctx **out, const mfc_grid *grid, int n_fluids, const mfc_fluid 
     if (grid->ndim < 1 || grid->ndim > 3 || n_fluids < 1) return MFC_EINVAL;
     if (n_fluids > MFC_MAX_FLUIDS) return MFC_EUNSUPPORTED;
     if (opts && opts->kapila && n_fluids != 2) return MFC_EUNSUPPORTED;
+    const int order = (opts && opts->weno_order != 0) ? opts->weno_order : 5;
+    if (order != 1 && order != 3 && order != 5) return MFC_EINVAL;
     for (int d = 0; d < grid->ndim; ++d) {
         if (grid->n[d] < MFC_NG || !(grid->hi[d] > grid->lo[d])) return MFC_EINVAL;
         if (bc->lo[d] != MFC_BC_PERIODIC && bc->lo[d] != MFC_BC_EXTRAP) return MFC_EINVAL;
@@ -270,6 +272,7 @@ int mfc_init(mfc_ctx **out, const mfc_grid *grid, int n_fluids, const mfc_fluid 
     c->neq = 2 * n_fluids + grid->ndim;
     c->device = dev;
     c->cfl = (opts && opts->cfl > 0.0) ? opts->cfl : 0.3;
+    c->order = order;
     const double eps = (opts && opts->weno_eps > 0.0) ? opts->weno_eps : 1.0e-16;
 
     Geo &g = c->g;
@@ -433,7 +436,7 @@ int mfc_line_fluxes(mfc_ctx *c, int dir, int n, const double *w_dev, double *vL_
     if (!c || !w_dev || !vL_dev || !vR_dev || !F_dev || !uface_dev || n < 1 || dir < 0 || dir >= c->ndim) return MFC_EINVAL;
     DeviceGuard guard(c->device);
     c->launch_total += 2;
-    return cuda_to_status(launch_line(c->ndim, c->nf, dir, c->e, n, w_dev, vL_dev, vR_dev, F_dev, uface_dev, (cudaStream_t)stream));
+    return cuda_to_status(launch_line(c->ndim, c->nf, c->order, dir, c->e, n, w_dev, vL_dev, vR_dev, F_dev, uface_dev, (cudaStream_t)stream));
 }
 
 int mfc_profile_enable(mfc_ctx *c, int on)

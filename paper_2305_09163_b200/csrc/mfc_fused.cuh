@@ -100,7 +100,7 @@ struct NoHook {
 // `early` runs at the top of the first FP64-heavy block and `mid` at the top of the second: the caller's loads,
 // cp.async issues and the cons->prim chains of the NEXT plane go there, so that they overlap this plane's
 // arithmetic instead of forming latency-bound phases of their own.
-template <int D, int NF, int TY, class Early = NoHook, class Mid = NoHook>
+template <int D, int NF, int TY, int ORDER, class Early = NoHook, class Mid = NoHook>
 __device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, const Eos &eos, double cx, double cy,
                                            double (&acc)[2 * NF + D], Early early = Early(), Mid mid = Mid())
 {
@@ -138,14 +138,14 @@ __device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, cons
 #pragma unroll
                 for (int e = 0; e < NEQ; ++e) {
                     const double *s5 = pb + e * PPL;
-                    weno5(s5[0], s5[-st] - s5[-2 * st], s5[0] - s5[-st], s5[st] - s5[0], s5[2 * st] - s5[st], eos.weno_eps4, v, unused);
+                    reconstruct<ORDER>(s5[0], s5[-st] - s5[-2 * st], s5[0] - s5[-st], s5[st] - s5[0], s5[2 * st] - s5[st], eos.weno_eps4, v, unused);
                     dst[e * ds] = v;
                 }
             } else {
 #pragma unroll
                 for (int e = 0; e < NEQ; ++e) {
                     const double *s5 = pb + e * PPL;
-                    weno5(s5[0], s5[-st] - s5[-2 * st], s5[0] - s5[-st], s5[st] - s5[0], s5[2 * st] - s5[st], eos.weno_eps4, unused, v);
+                    reconstruct<ORDER>(s5[0], s5[-st] - s5[-2 * st], s5[0] - s5[-st], s5[st] - s5[0], s5[2 * st] - s5[st], eos.weno_eps4, unused, v);
                     dst[e * ds] = v;
                 }
             }
@@ -159,7 +159,7 @@ __device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, cons
 #pragma unroll
         for (int e = 0; e < NEQ; ++e) {
             const double *s5 = pc + e * PPL;
-            weno5(s5[0], s5[-FPX] - s5[-2 * FPX], s5[0] - s5[-FPX], s5[FPX] - s5[0], s5[2 * FPX] - s5[FPX], eos.weno_eps4, vLy[e], vRy[e]);
+            reconstruct<ORDER>(s5[0], s5[-FPX] - s5[-2 * FPX], s5[0] - s5[-FPX], s5[FPX] - s5[0], s5[2 * FPX] - s5[FPX], eos.weno_eps4, vLy[e], vRy[e]);
         }
 #pragma unroll
         for (int e = 0; e < NEQ; ++e) B.X[e * NT + tid] = vRy[e];
@@ -174,7 +174,7 @@ __device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, cons
 #pragma unroll
         for (int e = 0; e < NEQ; ++e) {
             const double *s5 = pc + e * PPL;
-            weno5(s5[0], s5[-1] - s5[-2], s5[0] - s5[-1], s5[1] - s5[0], s5[2] - s5[1], eos.weno_eps4, vL[e], vR[e]);
+            reconstruct<ORDER>(s5[0], s5[-1] - s5[-2], s5[0] - s5[-1], s5[1] - s5[0], s5[2] - s5[1], eos.weno_eps4, vL[e], vR[e]);
         }
 #pragma unroll
         for (int e = 0; e < NEQ; ++e) {
@@ -267,7 +267,7 @@ __device__ __forceinline__ long long staged_source(const Geo &g, int x0, int y0,
 // ---------------------------------------------------------------------------------------------------------
 // 1D and 2D: one tile per block
 // ---------------------------------------------------------------------------------------------------------
-template <int D, int NF, int TY>
+template <int D, int NF, int TY, int ORDER>
 __global__ void __launch_bounds__(FTX *TY, 1)
     rhs_fused_plane_kernel(Geo g, Eos eos, const double *__restrict__ q, SweepOut o, int ntx)
 {
@@ -301,7 +301,7 @@ __global__ void __launch_bounds__(FTX *TY, 1)
     double acc[NEQ];
 #pragma unroll
     for (int e = 0; e < NEQ; ++e) acc[e] = 0.0;
-    inplane_xy<D, NF, TY>(B, eos, o.coef * g.inv_dx[0], D >= 2 ? o.coef * g.inv_dx[1] : 0.0, acc);
+    inplane_xy<D, NF, TY, ORDER>(B, eos, o.coef * g.inv_dx[0], D >= 2 ? o.coef * g.inv_dx[1] : 0.0, acc);
     if (active) {
 #pragma unroll
         for (int e = 0; e < NEQ; ++e) {
@@ -316,7 +316,7 @@ __global__ void __launch_bounds__(FTX *TY, 1)
 // ---------------------------------------------------------------------------------------------------------
 // 3D: tile in (x, y), march along z
 // ---------------------------------------------------------------------------------------------------------
-template <int NF, int TY>
+template <int NF, int TY, int ORDER>
 __global__ void __launch_bounds__(FTX *TY, 1)
     rhs_fused_march_kernel(Geo g, Eos eos, const double *__restrict__ q, SweepOut o, int ntx, int nty, int seg)
 {
@@ -466,7 +466,7 @@ __global__ void __launch_bounds__(FTX *TY, 1)
                 convert_staged(true, next_inplane ? ip + 1 : -1);
             };
             const InplaneBufs<D, NF, TY> B(P, rim, R + ((m + 1) & 3) * NEQ * NT, X8);
-            inplane_xy<D, NF, TY>(B, eos, cx, cy, acc, early, mid);
+            inplane_xy<D, NF, TY, ORDER>(B, eos, cx, cy, acc, early, mid);
         } else {
             cp_async_wait<1>();
             convert_staged(true, next_inplane ? ip + 1 : -1);
@@ -534,7 +534,7 @@ __global__ void __launch_bounds__(FTX *TY, 1)
 #pragma unroll
                 for (int e = 0; e < NEQ; ++e) {
                     const double vc = rc[e * NT], vd = rd[e * NT];
-                    weno5(vc, vb[e] - vprev[e], vc - vb[e], vd - vc, wn[e] - vd, eos.weno_eps4, vL[e], vR[e]);
+                    reconstruct<ORDER>(vc, vb[e] - vprev[e], vc - vb[e], vd - vc, wn[e] - vd, eos.weno_eps4, vL[e], vR[e]);
                 }
 #pragma unroll
                 for (int e = 0; e < NEQ; ++e) park[e * NT + tid] = vL[e];

@@ -14,6 +14,14 @@
 
 namespace mfc {
 
+#define MFC_FOR_ORDER(order, STMT)                                                                                    \
+    switch (order) {                                                                                                  \
+        case 1: { constexpr int ORDER = 1; STMT; } break;                                                             \
+        case 3: { constexpr int ORDER = 3; STMT; } break;                                                             \
+        case 5: { constexpr int ORDER = 5; STMT; } break;                                                             \
+        default: return cudaErrorInvalidValue;                                                                        \
+    }
+
 #define MFC_FOR_NF(nf, STMT)                                                                                          \
     switch (nf) {                                                                                                     \
         case 1: { constexpr int NF = 1; STMT; } break;                                                                \
@@ -59,7 +67,7 @@ static int fused_segment(const Geo &g, long long tiles, int wanted)
     return best_seg;
 }
 
-template <int D, int NF>
+template <int D, int NF, int ORDER>
 static void launch_fused(const Geo &g, const Eos &e, const double *q, const SweepOut &o, int segment, cudaStream_t s)
 {
     constexpr int TY = fused_ty<D, NF>();
@@ -70,20 +78,29 @@ static void launch_fused(const Geo &g, const Eos &e, const double *q, const Swee
     if constexpr (D == 3) {
         const int seg = fused_segment(g, (long long)ntx * nty, segment);
         const int nseg = (g.n[2] + seg - 1) / seg;
-        cudaFuncSetAttribute(rhs_fused_march_kernel<NF, TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::bytes);
-        rhs_fused_march_kernel<NF, TY><<<(unsigned)((long long)ntx * nty * nseg), C::NT, C::bytes, s>>>(g, e, q, o, ntx, nty, seg);
+        cudaFuncSetAttribute(rhs_fused_march_kernel<NF, TY, ORDER>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::bytes);
+        rhs_fused_march_kernel<NF, TY, ORDER><<<(unsigned)((long long)ntx * nty * nseg), C::NT, C::bytes, s>>>(g, e, q, o, ntx, nty, seg);
     } else {
-        cudaFuncSetAttribute(rhs_fused_plane_kernel<D, NF, TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::bytes);
-        rhs_fused_plane_kernel<D, NF, TY><<<(unsigned)((long long)ntx * nty), C::NT, C::bytes, s>>>(g, e, q, o, ntx);
+        cudaFuncSetAttribute(rhs_fused_plane_kernel<D, NF, TY, ORDER>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::bytes);
+        rhs_fused_plane_kernel<D, NF, TY, ORDER><<<(unsigned)((long long)ntx * nty), C::NT, C::bytes, s>>>(g, e, q, o, ntx);
     }
 }
 
-cudaError_t MFC_CAT(launch_rhs_d, MFC_D)(int nf, const Geo &g, const Eos &e, const double *q, const SweepOut &o, int segment,
-                                         cudaStream_t s)
+template <int D, int NF>
+static cudaError_t launch_fused_order(int order, const Geo &g, const Eos &e, const double *q, const SweepOut &o, int segment,
+                                      cudaStream_t s)
+{
+    MFC_FOR_ORDER(order, (launch_fused<D, NF, ORDER>(g, e, q, o, segment, s)))
+    return cudaSuccess;
+}
+
+cudaError_t MFC_CAT(launch_rhs_d, MFC_D)(int nf, int order, const Geo &g, const Eos &e, const double *q, const SweepOut &o,
+                                         int segment, cudaStream_t s)
 {
     constexpr int D = MFC_D;
-    MFC_FOR_NF(nf, (launch_fused<D, NF>(g, e, q, o, segment, s)))
-    return cudaGetLastError();
+    cudaError_t err = cudaSuccess;
+    MFC_FOR_NF(nf, (err = launch_fused_order<D, NF>(order, g, e, q, o, segment, s)))
+    return err != cudaSuccess ? err : cudaGetLastError();
 }
 
 cudaError_t MFC_CAT(launch_cfl_d, MFC_D)(int nf, const Geo &g, const Eos &e, const double *q, unsigned long long *min_bits,
@@ -98,23 +115,25 @@ cudaError_t MFC_CAT(launch_cfl_d, MFC_D)(int nf, const Geo &g, const Eos &e, con
 }
 
 template <int D, int NF, int DIR>
-static void launch_line_t(const Eos &e, int n, const double *w, double *vL, double *vR, double *F, double *uf, cudaStream_t s)
+static cudaError_t launch_line_t(int order, const Eos &e, int n, const double *w, double *vL, double *vR, double *F, double *uf,
+                                 cudaStream_t s)
 {
-    line_weno_kernel<D, NF, DIR><<<(n + 2 + 127) / 128, 128, 0, s>>>(e, n, w, vL, vR);
+    MFC_FOR_ORDER(order, (line_weno_kernel<D, NF, DIR, ORDER><<<(n + 2 + 127) / 128, 128, 0, s>>>(e, n, w, vL, vR)))
     line_hllc_kernel<D, NF, DIR><<<(n + 1 + 127) / 128, 128, 0, s>>>(e, n, vL, vR, F, uf);
+    return cudaSuccess;
 }
 
-cudaError_t MFC_CAT(launch_line_d, MFC_D)(int nf, int dir, const Eos &e, int n, const double *w, double *vL, double *vR,
+cudaError_t MFC_CAT(launch_line_d, MFC_D)(int nf, int order, int dir, const Eos &e, int n, const double *w, double *vL, double *vR,
                                           double *F, double *uf, cudaStream_t s)
 {
     constexpr int D = MFC_D;
     if (dir < 0 || dir >= D) return cudaErrorInvalidValue;
-    if (dir == 0) { MFC_FOR_NF(nf, (launch_line_t<D, NF, 0>(e, n, w, vL, vR, F, uf, s))) }
+    if (dir == 0) { MFC_FOR_NF(nf, (launch_line_t<D, NF, 0>(order, e, n, w, vL, vR, F, uf, s))) }
 #if MFC_D >= 2
-    else if (dir == 1) { MFC_FOR_NF(nf, (launch_line_t<D, NF, 1>(e, n, w, vL, vR, F, uf, s))) }
+    else if (dir == 1) { MFC_FOR_NF(nf, (launch_line_t<D, NF, 1>(order, e, n, w, vL, vR, F, uf, s))) }
 #endif
 #if MFC_D >= 3
-    else if (dir == 2) { MFC_FOR_NF(nf, (launch_line_t<D, NF, 2>(e, n, w, vL, vR, F, uf, s))) }
+    else if (dir == 2) { MFC_FOR_NF(nf, (launch_line_t<D, NF, 2>(order, e, n, w, vL, vR, F, uf, s))) }
 #endif
     return cudaGetLastError();
 }

@@ -72,7 +72,7 @@ __global__ void __launch_bounds__(256) cfl_kernel(Geo g, Eos eos, const double *
 // ---------------------------------------------------------------------------------------------------------
 // a2 + a3 on one line of primitives (stage parity): same weno5 / hllc as the sweeps, one thread per cell.
 // ---------------------------------------------------------------------------------------------------------
-template <int D, int NF, int DIR>
+template <int D, int NF, int DIR, int ORDER>
 __global__ void line_weno_kernel(Eos eos, int n, const double *__restrict__ w, double *vL, double *vR)
 {
     using I = Idx<D, NF>;
@@ -83,7 +83,7 @@ __global__ void line_weno_kernel(Eos eos, int n, const double *__restrict__ w, d
     for (int e = 0; e < I::NEQ; ++e) {
         const double *p = w + (long long)e * np + (t - 1 + NG);
         double l, r;
-        weno5(p[0], p[-1] - p[-2], p[0] - p[-1], p[1] - p[0], p[2] - p[1], eos.weno_eps4, l, r);
+        reconstruct<ORDER>(p[0], p[-1] - p[-2], p[0] - p[-1], p[1] - p[0], p[2] - p[1], eos.weno_eps4, l, r);
         vL[(long long)e * (n + 2) + t] = l;
         vR[(long long)e * (n + 2) + t] = r;
     }

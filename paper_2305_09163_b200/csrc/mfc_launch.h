@@ -48,22 +48,22 @@ struct SweepOut {
 };
 
 cudaError_t launch_prim(int ndim, int nf, const Geo &g, const Eos &e, const double *q, double *w, cudaStream_t s);
-cudaError_t launch_rhs(int ndim, int nf, const Geo &g, const Eos &e, const double *q, const SweepOut &o, int segment,
+cudaError_t launch_rhs(int ndim, int nf, int order, const Geo &g, const Eos &e, const double *q, const SweepOut &o, int segment,
                        cudaStream_t s);
 cudaError_t launch_cfl(int ndim, int nf, const Geo &g, const Eos &e, const double *q, unsigned long long *min_bits,
                        cudaStream_t s);
 cudaError_t launch_eos_seed(const double *gm1_dev, double *ygm1_dev, int n, cudaStream_t s);
-cudaError_t launch_line(int ndim, int nf, int dir, const Eos &e, int n, const double *w, double *vL, double *vR,
+cudaError_t launch_line(int ndim, int nf, int order, int dir, const Eos &e, int n, const double *w, double *vL, double *vR,
                         double *F, double *uf, cudaStream_t s);
 
 // per-dimension implementations
 #define MFC_DECL_DIM(D)                                                                                               \
     cudaError_t launch_prim_d##D(int nf, const Geo &g, const Eos &e, const double *q, double *w, cudaStream_t s);     \
-    cudaError_t launch_rhs_d##D(int nf, const Geo &g, const Eos &e, const double *q, const SweepOut &o, int segment,  \
+    cudaError_t launch_rhs_d##D(int nf, int order, const Geo &g, const Eos &e, const double *q, const SweepOut &o, int segment,  \
                                 cudaStream_t s);                                                                      \
     cudaError_t launch_cfl_d##D(int nf, const Geo &g, const Eos &e, const double *q, unsigned long long *min_bits,    \
                                 cudaStream_t s);                                                                      \
-    cudaError_t launch_line_d##D(int nf, int dir, const Eos &e, int n, const double *w, double *vL, double *vR,       \
+    cudaError_t launch_line_d##D(int nf, int order, int dir, const Eos &e, int n, const double *w, double *vL, double *vR,       \
                                  double *F, double *uf, cudaStream_t s);
 MFC_DECL_DIM(1)
 MFC_DECL_DIM(2)

@@ -52,6 +52,7 @@ class Problem:
     steps: int = 1
     seed: int | None = None
     notes: str = ""
+    weno_order: int = 5  # 5: WENO5-JS (the paper's default), 3: WENO3-JS, 1: piecewise constant
     kapila: bool = False  # K div(u) source of PAPER.md Eq. 2 on the alpha row (two fluids); False = Allaire
 
     @property

@@ -53,6 +53,8 @@ def test_strerror_and_version(lib):
     (dict(bc_lo=(0,), bc_hi=(1,)), B.MFC_EINVAL),                        # periodic on one side only
     (dict(bc_lo=(7,), bc_hi=(7,)), B.MFC_EINVAL),
     (dict(lo=(1.0,), hi=(1.0,)), B.MFC_EINVAL),
+    (dict(weno_order=4), B.MFC_EINVAL),                                   # reconstruction order 1, 3 or 5
+    (dict(weno_order=7), B.MFC_EINVAL),
     (dict(fluids=[(1.4, 0.0)], kapila=True), B.MFC_EUNSUPPORTED),         # Eq. 2 is the two-fluid coefficient
     (dict(fluids=[(4.4, 6e8), (1.4, 0.0), (1.33, 0.0)], kapila=True), B.MFC_EUNSUPPORTED),
 ])

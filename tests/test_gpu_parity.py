@@ -187,6 +187,45 @@ def test_uniform_state_has_exactly_zero_rhs_on_gpu(ndim, nf, periodic):
     assert np.all(got[it] == 0.0)
 
 
+# Lower-order reconstructions: same parity bars with opts.weno_order = 3, 1
+@pytest.mark.parametrize("order", [1, 3])
+@pytest.mark.parametrize("ndim,nf,periodic", [(1, 2, False), (2, 2, True), (2, 1, False), (3, 2, False), (3, 3, True), (3, 1, True)])
+def test_rhs_parity_lower_order_reconstruction(order, ndim, nf, periodic):
+    import dataclasses
+    prob, q = wl.random_state(ndim, SIZES[ndim], nf, seed=50 + 3 * ndim + nf, periodic=periodic)
+    prob = dataclasses.replace(prob, weno_order=order)
+    check_rhs(prob, q, march_segment=8)
+    with Gpu(prob) as g1, Gpu(dataclasses.replace(prob, weno_order=5)) as g5:       # the option is really on
+        it = prob.interior()
+        assert not np.allclose(g1.rhs(q)[it], g5.rhs(q)[it], rtol=1e-6)
+
+
+@pytest.mark.parametrize("order", [1, 3])
+def test_rk3_parity_lower_order_reconstruction(order):
+    import dataclasses
+    prob, q = wl.random_state(3, (40, 29, 33), 2, seed=92, periodic=True, rough=False)
+    check_rk(dataclasses.replace(prob, weno_order=order), q, march_segment=8)
+
+
+@pytest.mark.parametrize("order", [1, 3])
+def test_line_states_lower_order_reconstruction(order):
+    import dataclasses
+    prob, _ = wl.random_state(2, (8, 8), 2, seed=1)
+    prob = dataclasses.replace(prob, weno_order=order)
+    orc = oracle.Oracle(prob)
+    rng = np.random.default_rng(order)
+    w = random_prim_line(prob, 333, rng, False)
+    rL, rR, rF, ru = orc.line(1, w)
+    with Gpu(prob) as g:
+        gL, gR, gF, gu = g.line(1, w)
+    for e in range(prob.neq):
+        s = np.max(np.abs(w[e])) + 1e-300
+        assert np.max(np.abs(gL[e] - rL[e])) <= 1e-13 * s and np.max(np.abs(gR[e] - rR[e])) <= 1e-13 * s
+        assert np.max(np.abs(gF[e] - rF[e])) <= 1e-11 * (np.max(np.abs(rF[e])) + 1e-300)
+    if order == 1:                                                  # piecewise constant: the states are the cell values
+        assert np.array_equal(gL, w[:, 2:-2]) and np.array_equal(gR, w[:, 2:-2])
+
+
 # Kapila source: same parity bar with opts.kapila on
 @pytest.mark.parametrize("ndim", [1, 2, 3])
 @pytest.mark.parametrize("periodic", [True, False])

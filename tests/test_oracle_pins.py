@@ -586,3 +586,105 @@ def test_kapila_changes_nothing_where_the_velocity_is_uniform():
     L0 = interior(prob, oracle.Oracle(prob).rhs(q.copy()))
     L1 = interior(prob, oracle.Oracle(_kapila(prob)).rhs(q.copy()))
     assert np.allclose(L0[-1], L1[-1], rtol=0, atol=1e-9 * np.max(np.abs(L0[-1])))
+
+
+# ---------------------------------------------------------------------------------------------
+# Lower-order reconstructions (Eq. 12 with k = 2, k = 1)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("deg", [0, 1])
+def test_weno3_exact_for_linear_data_any_weights(deg):
+    rng = np.random.default_rng(deg + 7)
+    for _ in range(50):
+        poly = Polynomial(rng.normal(size=deg + 1))
+        h, x0 = rng.uniform(0.05, 2.0), rng.normal()
+        a = _cell_averages(poly, x0 + h * np.arange(-1, 2), h)
+        vL, vR = oracle.weno3(*a, eps=1e-16)
+        scale = np.max(np.abs(a)) + 1e-300
+        assert abs(vL - poly(x0 + h / 2)) <= 1e-14 * scale
+        assert abs(vR - poly(x0 - h / 2)) <= 1e-14 * scale
+
+
+def test_weno3_exact_for_quadratics_at_ideal_weights_only():
+    """Ideal weights (1/3, 2/3) reproduce the 3-cell quadratic (third order); the JS weights do not."""
+    rng = np.random.default_rng(11)
+    worst_js = 0.0
+    for _ in range(50):
+        poly = Polynomial(rng.normal(size=3))
+        h, x0 = rng.uniform(0.1, 1.0), rng.normal()
+        a = _cell_averages(poly, x0 + h * np.arange(-1, 2), h)
+        vL, vR = oracle.weno3(*a, eps=1e40)
+        scale = np.max(np.abs(a))
+        assert abs(vL - poly(x0 + h / 2)) <= 1e-13 * scale
+        assert abs(vR - poly(x0 - h / 2)) <= 1e-13 * scale
+        jL, _ = oracle.weno3(*a, eps=1e-16)
+        worst_js = max(worst_js, abs(jL - poly(x0 + h / 2)) / scale)
+    assert worst_js > 1e-6
+
+
+def test_weno3_mirror_symmetry_and_smooth_stencil_at_a_step():
+    rng = np.random.default_rng(5)
+    for _ in range(20):
+        b, c, d = rng.normal(size=3)
+        vL, vR = oracle.weno3(b, c, d)
+        mL, mR = oracle.weno3(d, c, b)
+        assert vL == mR and vR == mL
+    # step between cells i and i+1: the left state at i+1/2 comes from the smooth pair (i-1, i), not across the jump
+    vL, _ = oracle.weno3(1.0, 1.0 + 1e-3, 50.0)
+    assert abs(vL - (1.0 + 1.5e-3)) < 1e-6
+
+
+@pytest.mark.parametrize("order,eps,rate", [(1, 1e-16, 1.0), (3, 1e40, 3.0), (3, 1e-16, None)])
+def test_lower_order_smooth_advection_converges_at_its_order(order, eps, rate):
+    """Same experiment as C3 (1-D two-fluid advection of a smooth alpha profile at constant u, p), a fraction of a
+    period with dt ~ dx^(5/3) so that RK3 does not mask the spatial order.  Third order is the DESIGN order of
+    WENO3, reached with the ideal weights (eps huge); with eps = 1e-16 the Jiang-Shu weights of the 3-point scheme
+    are known to fall to about first order in the maximum norm at the critical points of the profile, so that case
+    only checks convergence and that the error is no better than the ideal-weight one."""
+    import dataclasses
+    errs = []
+    for n in (40, 80, 160):
+        prob, _ = wl.random_state(1, (n,), 2, seed=1, periodic=True)
+        prob = dataclasses.replace(prob, weno_order=order, weno_eps=eps)
+        x = prob.centers(0)[None, None, :]
+        h = prob.dx[0]
+        # cell averages of alpha = 0.5 + 0.3 sin(2 pi x)
+        a = 0.5 + 0.3 * (np.cos(2 * np.pi * (x - h / 2)) - np.cos(2 * np.pi * (x + h / 2))) / (2 * np.pi * h)
+        one = np.ones_like(x)
+        u0, p0 = 100.0, 1.0e5
+        q = wl.assemble(prob, [a, 1 - a], [1000 * one, 1000 * one], [u0 * one], p0 * one)
+        orc = oracle.Oracle(prob)
+        T, t = 0.1 / u0, 0.0
+        dt = 0.2 * h / u0 * (h * 40) ** (2.0 / 3.0)
+        while t < T - 1e-15:
+            step = min(dt, T - t)
+            orc.rk3_step(q, step)
+            t += step
+        xs = x - u0 * T
+        exact = 0.5 + 0.3 * (np.cos(2 * np.pi * (xs - h / 2)) - np.cos(2 * np.pi * (xs + h / 2))) / (2 * np.pi * h)
+        errs.append(np.max(np.abs(interior(prob, q)[-1] - exact)))
+    rates = np.log2(np.array(errs[:-1]) / np.array(errs[1:]))
+    if rate is None:
+        assert np.all(rates > 0.9) and errs[-1] > 1e-5, (rates, errs)
+    else:
+        assert np.all(np.abs(rates - rate) < 0.3), (order, rates, errs)
+
+
+@pytest.mark.parametrize("order", [1, 3])
+def test_lower_order_uniform_state_and_conservation(order):
+    import dataclasses
+    prob, q = wl.random_state(2, (14, 11), 2, seed=3, periodic=True)
+    prob = dataclasses.replace(prob, weno_order=order)
+    orc = oracle.Oracle(prob)
+    L = interior(prob, orc.rhs(q.copy()))
+    for k in range(prob.nf + prob.ndim + 1):                        # conservative rows sum to round-off
+        assert abs(np.sum(L[k])) <= 1e-11 * np.sum(np.abs(L[k]))
+    it = prob.interior()
+    qu = q.copy()
+    qu[it] = qu[it][:, :1, :1, :1]
+    assert np.all(interior(prob, orc.rhs(qu)) == 0.0)
+    # first order: the face states are the cell values
+    if order == 1:
+        w = orc.cons_to_prim(q.copy())
+        line = np.ascontiguousarray(w[:, 0, 5, :])
+        vL, vR, F, uf = orc.line(0, line)
+        assert np.array_equal(vL[:, 1:-1], line[:, 3:-3]) and np.array_equal(vR[:, 1:-1], line[:, 3:-3])
