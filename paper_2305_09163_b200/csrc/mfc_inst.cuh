@@ -6,6 +6,8 @@
 #ifndef MFC_D
 #error "define MFC_D (1, 2 or 3) before including mfc_inst.cuh"
 #endif
+// rows of the 3D tile for up to two fluids (a multiple of 4: one warp per scheduler and group); -DMFC_TY_2F=8 builds
+// the 8-row variant measured in DESIGN.md 6.1
 #ifndef MFC_TY_2F
 #define MFC_TY_2F (NF <= 2 ? 12 : 8)
 #endif
