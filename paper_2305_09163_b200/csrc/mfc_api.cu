@@ -194,7 +194,7 @@ int rk3(mfc_ctx *c, double *q, double dt, cudaStream_t s)
 
 int cfl_dt(mfc_ctx *c, const double *q, double *dt_host, cudaStream_t s)
 {
-    if (cudaMemsetAsync(c->min_dev, 0x7f, sizeof(unsigned long long), s) != cudaSuccess) return MFC_ECUDA;
+    if (cudaMemsetAsync(c->min_dev, 0, sizeof(unsigned long long), s) != cudaSuccess) return MFC_ECUDA;   // max of speeds / dx
     cudaError_t err;
     {
         Timed t(c, MFC_K_CFL, s);
@@ -206,7 +206,7 @@ int cfl_dt(mfc_ctx *c, const double *q, double *dt_host, cudaStream_t s)
     if (cudaStreamSynchronize(s) != cudaSuccess) return MFC_ECUDA;
     double v;
     std::memcpy(&v, c->min_host, sizeof(double));
-    *dt_host = c->cfl * v;
+    *dt_host = c->cfl * (1.0 / v);   // v = max over cells and directions of (|u_d| + c) / dx_d
     return MFC_OK;
 }
 

@@ -111,7 +111,7 @@ cudaError_t MFC_CAT(launch_cfl_d, MFC_D)(int nf, const Geo &g, const Eos &e, con
     constexpr int D = MFC_D;
     const long long ncell = (long long)g.n[0] * g.n[1] * g.n[2];
     long long want = (ncell + 255) / 256;
-    const unsigned blocks = (unsigned)(want < 148 * 8 ? (want < 1 ? 1 : want) : 148 * 8);
+    const unsigned blocks = (unsigned)(want < 148 * 16 ? (want < 1 ? 1 : want) : 148 * 16);
     MFC_FOR_NF(nf, (cfl_kernel<D, NF><<<blocks, 256, 0, s>>>(g, e, q, min_bits)))
     return cudaGetLastError();
 }
