@@ -374,6 +374,13 @@ def test_rk3_parity_cfg4_reduced():
     check_rk(prob, q)
 
 
+def test_rk3_full_size_cfg3_whole_state():
+    """The headline workload at its full size, in the launch configuration bench.py times (default segment heuristic):
+    two complete steps (CFL + 3 stages each) compared cell by cell with the oracle over the whole 256^3 state."""
+    prob, q = wl.cfg3()
+    check_rk(prob, q, steps=2)
+
+
 def test_single_stage_combination_matches_forward_euler_of_rhs():
     """q + dt L(q) assembled by the last sweep equals the separately returned L (same kernels, two output modes)."""
     prob, q = wl.random_state(3, (30, 20, 25), 2, seed=9, periodic=True)
