@@ -374,6 +374,21 @@ def test_rk3_parity_cfg4_reduced():
     check_rk(prob, q)
 
 
+def test_results_are_bitwise_reproducible_from_run_to_run():
+    """A data race between the warps of a block (exchange buffers, ring slots, staged plane) would show up as run-to-run
+    differences: the same five steps, three times, must give the same bits (compute-sanitizer is not available on the
+    GPU pool, so this and the parity tests are the race checks)."""
+    prob, q = wl.random_state(3, (97, 50, 41), 2, seed=123, periodic=False)
+    orc = oracle.Oracle(prob)
+    dts = [0.5 * orc.cfl_dt(q.copy(), prob.cfl)] * 5
+    runs = []
+    for _ in range(3):
+        with Gpu(prob) as g:
+            runs.append(g.rk3(q, dts))
+    assert np.array_equal(runs[0], runs[1]) and np.array_equal(runs[0], runs[2])
+    assert np.all(np.isfinite(runs[0][prob.interior()]))
+
+
 def test_rk3_full_size_cfg3_whole_state():
     """The headline workload at its full size, in the launch configuration bench.py times (default segment heuristic):
     two complete steps (CFL + 3 stages each) compared cell by cell with the oracle over the whole 256^3 state."""
