@@ -65,7 +65,7 @@ struct FusedCfg {
     // ring (4 slots) + parked left state + staging of raw q: own column of the next plane, q_s of the cell being
     // written, halo cells of the next two staged planes (double buffer)
     static constexpr int nX = D == 2 ? NEQ * NT : 0;
-    static constexpr int nR = D == 3 ? 5 * NEQ * NT : 0;
+    static constexpr int nR = D == 3 ? NEQ * NT + 2 : 0;            // y exchange buffer + the TMEM base word (ring, park: in TMEM)
     static constexpr int nS = D == 3 ? NEQ * (2 * NT + 2 * NH) : 0;
     static constexpr int doubles = nP + nHx + nHy + nX8 + nX + nR + nS;
     static constexpr int bytes = doubles * (int)sizeof(double);
@@ -314,6 +314,67 @@ __global__ void __launch_bounds__(FTX *TY, 1)
 }
 
 // ---------------------------------------------------------------------------------------------------------
+// Tensor memory (TMEM, 256 KB per SM) as thread-private scratch.  Nothing on this path uses the tensor cores, so
+// the whole of it is free: the z window of a column (ring of primitive planes), the parked left state, the
+// previous z flux and the plane that left the ring live there instead of in shared memory and registers.
+// A warp reaches the 32 TMEM lanes of its quarter (warp index mod 4), one lane per thread; the warps of a quarter
+// take disjoint column ranges.  tcgen05.ld / st with shape 32x32b move N consecutive 32-bit columns of the
+// thread's own lane to / from registers.  TV = values (doubles) per transfer: 8 (x16) or 16 (x32).
+// ---------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void tmem_alloc512(unsigned *smem_word)
+{
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"((unsigned)__cvta_generic_to_shared(smem_word)) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc512(unsigned base)
+{
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(base) : "memory");
+}
+template <int TV>
+__device__ __forceinline__ void tmem_load(unsigned a, double (&v)[TV])
+{
+    static_assert(TV == 8 || TV == 16, "8 or 16 doubles per transfer");
+    unsigned r[2 * TV];
+    if constexpr (TV == 8) {
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                     : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+                       "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+                     : "r"(a));
+    } else {
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
+                     : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+                       "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]),
+                       "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]),
+                       "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+                     : "r"(a));
+    }
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+    for (int k = 0; k < TV; ++k) v[k] = __hiloint2double((int)r[2 * k + 1], (int)r[2 * k]);
+}
+template <int TV>
+__device__ __forceinline__ void tmem_store(unsigned a, const double (&v)[TV])
+{
+    unsigned r[2 * TV];
+#pragma unroll
+    for (int k = 0; k < TV; ++k) { r[2 * k] = (unsigned)__double2loint(v[k]); r[2 * k + 1] = (unsigned)__double2hiint(v[k]); }
+    if constexpr (TV == 8) {
+        asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
+                     ::"r"(a), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]),
+                       "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
+                     : "memory");
+    } else {
+        asm volatile("tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31,%32};"
+                     ::"r"(a), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]),
+                       "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]), "r"(r[16]), "r"(r[17]),
+                       "r"(r[18]), "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]), "r"(r[24]), "r"(r[25]), "r"(r[26]),
+                       "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31])
+                     : "memory");
+    }
+    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+}
+
+// ---------------------------------------------------------------------------------------------------------
 // 3D: tile in (x, y), march along z
 // ---------------------------------------------------------------------------------------------------------
 template <int NF, int TY, int ORDER>
@@ -329,11 +390,15 @@ __global__ void __launch_bounds__(FTX *TY, 1)
     double *const P = sm;
     double *const rim = P + C::nP;
     double *const X8 = rim + C::nHx + C::nHy;
-    double *const R = X8 + C::nX8;                                  // [4][NEQ][NT] ring of primitive planes
-    double *const park = R + 4 * NEQ * NT;                          // [NEQ][NT]    left state of the next z face
-    double *const SQ = park + NEQ * NT;                             // [NEQ][NT]    raw q, own column, next plane
+    double *const X = X8 + C::nX8;                                  // [NEQ][NT]    y exchange
+    double *const SQ = X + NEQ * NT;                                // [NEQ][NT]    raw q, own column, next plane
     double *const SS = SQ + NEQ * NT;                               // [NEQ][NT]    raw q_s of the cell being written
     double *const SH = SS + NEQ * NT;                               // [2][NEQ][NH] raw q, halo cells of the next two staged planes
+    unsigned *const tmem_word = reinterpret_cast<unsigned *>(SH + 2 * NEQ * NH);
+    // thread-private TMEM scratch (see above): slots of TV doubles = 2 TV columns each
+    constexpr int TV = NEQ + 1 <= 8 ? 8 : 16;
+    enum { T_RING = 0, T_PARK = 4, T_PREV = 5, T_FLUX = 6, T_SLOTS = 7 };
+    static_assert(T_SLOTS * 2 * TV * ((TY + 3) / 4) <= 512, "TMEM columns");
 
     const int tid = threadIdx.x, i = tid & 31, j = tid >> 5;
     int b = blockIdx.x;
@@ -391,10 +456,22 @@ __global__ void __launch_bounds__(FTX *TY, 1)
         }
     };
 
-    double Fmz[NEQ], ufmz = 0.0;                                    // flux and face velocity of the previous z face
-    double vprev[NEQ];                                              // own cell of the plane that just left the ring
+    // TMEM: one warp allocates all 512 columns (one block per SM), everybody reads the base after a barrier
+    if (j == 0) tmem_alloc512(tmem_word);
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const unsigned tmem_base = *tmem_word;
+    // this thread's scratch: lane = 32 (warp mod 4) + lane id (implied by the 32x32b shape), columns by warp / 4
+    const unsigned tbase = tmem_base + ((unsigned)(32 * (j & 3)) << 16) + (unsigned)((j >> 2) * T_SLOTS * 2 * TV);
+    auto tslot = [&](int s) -> unsigned { return tbase + (unsigned)(s * 2 * TV); };
+    {   // previous z flux (T_FLUX: NEQ fluxes + the face velocity) and the plane that left the ring (T_PREV) start at zero
+        double z[TV];
 #pragma unroll
-    for (int e = 0; e < NEQ; ++e) { Fmz[e] = 0.0; vprev[e] = 0.0; }
+        for (int k = 0; k < TV; ++k) z[k] = 0.0;
+        tmem_store<TV>(tslot(T_FLUX), z);
+        tmem_store<TV>(tslot(T_PREV), z);
+    }
 
     // cons->prim of the staged raw values, in place and thread-private: own column of the next plane (SQ) and this
     // thread's halo cells of the next staged plane (SH)
@@ -465,7 +542,7 @@ __global__ void __launch_bounds__(FTX *TY, 1)
                 cp_async_wait<1>();
                 convert_staged(true, next_inplane ? ip + 1 : -1);
             };
-            const InplaneBufs<D, NF, TY> B(P, rim, R + ((m + 1) & 3) * NEQ * NT, X8);
+            const InplaneBufs<D, NF, TY> B(P, rim, X, X8);
             inplane_xy<D, NF, TY, ORDER>(B, eos, cx, cy, acc, early, mid);
         } else {
             cp_async_wait<1>();
@@ -487,20 +564,28 @@ __global__ void __launch_bounds__(FTX *TY, 1)
         }
         // plane m of the own column (primitives since the conversion above) and plane m - 3 = ip: the latter sits in P
         // when it has just been differenced in plane (its ring slot was the exchange buffer)
-        double wn[NEQ], vb[NEQ];
-        {
-            const double *const pb = inplane ? pcw : R + ((m + 1) & 3) * NEQ * NT + tid;
-            const int sb = inplane ? PPL : NT;
+        double wn[TV], vb[TV];
 #pragma unroll
-            for (int e = 0; e < NEQ; ++e) { wn[e] = SQ[e * NT + tid]; vb[e] = n >= 3 ? pb[e * sb] : 0.0; }
+        for (int k = NEQ; k < TV; ++k) { wn[k] = 0.0; vb[k] = 0.0; }
+#pragma unroll
+        for (int e = 0; e < NEQ; ++e) wn[e] = SQ[e * NT + tid];
+        if (inplane) {
+#pragma unroll
+            for (int e = 0; e < NEQ; ++e) vb[e] = pcw[e * PPL];
+        } else if (n >= 3) {
+            tmem_load<TV>(tslot(T_RING + ((m + 1) & 3)), vb);
+        } else {
+#pragma unroll
+            for (int e = 0; e < NEQ; ++e) vb[e] = 0.0;
         }
         // "glue": plane ip + 1 -> P, raw reads of the next iterations issued.  No FP64 work: half of the warps of every
         // scheduler run it BEFORE the z part and half AFTER it, so that it overlaps the other half's arithmetic
         auto glue = [&]() {
             if (next_inplane) {
-                const double *const rp = R + ((m + 2) & 3) * NEQ * NT + tid;  // plane m - 2 = ip + 1
+                double rp[TV];                                      // plane m - 2 = ip + 1
+                tmem_load<TV>(tslot(T_RING + ((m + 2) & 3)), rp);
 #pragma unroll
-                for (int e = 0; e < NEQ; ++e) pcw[e * PPL] = rp[e * NT];
+                for (int e = 0; e < NEQ; ++e) pcw[e * PPL] = rp[e];
                 const double *const sh = SH + ((ip + 1) & 1) * NEQ * NH;
 #pragma unroll
                 for (int t = 0; t < NHT; ++t) {
@@ -526,38 +611,41 @@ __global__ void __launch_bounds__(FTX *TY, 1)
             // ---- z: reconstruct cell m - 2, solve face (m - 2) - 1/2, difference for cell m - 3 = ip ----
             if (n >= 4) {
                 const int c = m - 2;
-                const double *const rc = R + ((m + 2) & 3) * NEQ * NT + tid;  // plane m - 2
-                const double *const rd = R + ((m + 3) & 3) * NEQ * NT + tid;  // plane m - 1
-                double vLp[NEQ], vL[NEQ], vR[NEQ];
+                double rc[TV], rd[TV], vLp[TV], vprev[TV], vL[TV], vR[NEQ];
+                tmem_load<TV>(tslot(T_RING + ((m + 2) & 3)), rc);   // plane m - 2
+                tmem_load<TV>(tslot(T_RING + ((m + 3) & 3)), rd);   // plane m - 1
+                tmem_load<TV>(tslot(T_PARK), vLp);
+                tmem_load<TV>(tslot(T_PREV), vprev);
 #pragma unroll
-                for (int e = 0; e < NEQ; ++e) vLp[e] = park[e * NT + tid];
+                for (int k = NEQ; k < TV; ++k) vL[k] = 0.0;
 #pragma unroll
-                for (int e = 0; e < NEQ; ++e) {
-                    const double vc = rc[e * NT], vd = rd[e * NT];
-                    reconstruct<ORDER>(vc, vb[e] - vprev[e], vc - vb[e], vd - vc, wn[e] - vd, eos.weno_eps4, vL[e], vR[e]);
-                }
-#pragma unroll
-                for (int e = 0; e < NEQ; ++e) park[e * NT + tid] = vL[e];
+                for (int e = 0; e < NEQ; ++e)
+                    reconstruct<ORDER>(rc[e], vb[e] - vprev[e], rc[e] - vb[e], rd[e] - rc[e], wn[e] - rd[e], eos.weno_eps4, vL[e], vR[e]);
+                tmem_store<TV>(tslot(T_PARK), vL);
                 if (c >= k0) {
-                    double Fp[NEQ], ufp;
-                    hllc<D, NF, 2>(vLp, vR, eos, Fp, ufp);
-                    const double du = ufp - ufmz;
+                    double Fm[TV], Fn[TV];                          // previous and new flux; entry NEQ is the face velocity
+                    tmem_load<TV>(tslot(T_FLUX), Fm);
+                    double Fp[NEQ], ufp, vl7[NEQ];
+#pragma unroll
+                    for (int e = 0; e < NEQ; ++e) vl7[e] = vLp[e];
+                    hllc<D, NF, 2>(vl7, vR, eos, Fp, ufp);
+                    const double du = ufp - Fm[NEQ];
+#pragma unroll
+                    for (int k = 0; k < TV; ++k) Fn[k] = 0.0;
 #pragma unroll
                     for (int e = 0; e < NEQ; ++e) {
-                        double rr = Fmz[e] - Fp[e];
+                        double rr = Fm[e] - Fp[e];
                         if (e >= I::A) rr = fma(alpha_div_coef<NF>(eos, vb[e], vb[I::E]), du, rr);
                         acc[e] = fma(cz, rr, acc[e]);               // meaningful when c > k0, i.e. when ip >= k0
-                        Fmz[e] = Fp[e];
+                        Fn[e] = Fp[e];
                     }
-                    ufmz = ufp;
+                    Fn[NEQ] = ufp;
+                    tmem_store<TV>(tslot(T_FLUX), Fn);
                 }
             }
-#pragma unroll
-            for (int e = 0; e < NEQ; ++e) vprev[e] = vb[e];
-            // plane m enters the ring: the slot of plane m - 4 (the previous iteration's exchange buffer)
-            double *const rs = R + (m & 3) * NEQ * NT + tid;
-#pragma unroll
-            for (int e = 0; e < NEQ; ++e) rs[e * NT] = wn[e];
+            tmem_store<TV>(tslot(T_PREV), vb);
+            // plane m enters the ring: the slot of plane m - 4
+            tmem_store<TV>(tslot(T_RING + (m & 3)), wn);
             // ---- a5: out = ca q_n + cb q_s + coef L ----
             if (inplane && active) {
 #pragma unroll
@@ -574,6 +662,7 @@ __global__ void __launch_bounds__(FTX *TY, 1)
         }
         __syncthreads();                                            // P is staged, the exchange buffer is free
     }
+    if (j == 0) tmem_dealloc512(tmem_base);
 }
 
 }  // namespace mfc
