@@ -64,8 +64,8 @@ struct FusedCfg {
     // 1D / 2D: the y exchange has its own buffer.  3D: it lives in the ring slot of the plane staged in P;
     // ring (4 slots) + parked left state + staging of raw q: own column of the next plane, q_s of the cell being
     // written, halo cells of the next two staged planes (double buffer)
-    static constexpr int nX = D == 2 ? NEQ * NT : 0;
-    static constexpr int nR = D == 3 ? NEQ * NT + 2 : 0;            // y exchange buffer + the TMEM base word (ring, park: in TMEM)
+    static constexpr int nX = D == 2 ? 2 * NEQ * NT : 0;
+    static constexpr int nR = D == 3 ? 2 * NEQ * NT + 2 : 0;        // y exchange buffers + the TMEM base word (ring, park: in TMEM)
     static constexpr int nS = D == 3 ? NEQ * (2 * NT + 2 * NH) : 0;
     static constexpr int doubles = nP + nHx + nHy + nX8 + nX + nR + nS;
     static constexpr int bytes = doubles * (int)sizeof(double);
@@ -75,9 +75,9 @@ struct FusedCfg {
 template <int D, int NF, int TY>
 struct InplaneBufs {
     const double *P;     // staged plane with halo
-    double *X, *X8;      // y exchange [NEQ][NT] and its face-velocity row [NT]
+    double *X, *X2, *X8; // y exchange: right states [NEQ][NT], fluxes [NEQ][NT] and their face-velocity row [NT]
     double *HxL, *ExR, *HxR, *ExF, *HyL, *HyR;
-    __device__ __forceinline__ InplaneBufs(double *P_, double *rim, double *X_, double *X8_) : P(P_), X(X_), X8(X8_)
+    __device__ __forceinline__ InplaneBufs(double *P_, double *rim, double *X_, double *X2_, double *X8_) : P(P_), X(X_), X2(X2_), X8(X8_)
     {
         constexpr int NEQ = 2 * NF + D;
         HxL = rim;                    // [NEQ][TY]   left state of face -1/2 (from cell -1)
@@ -91,7 +91,7 @@ struct InplaneBufs {
 
 // ---------------------------------------------------------------------------------------------------------
 // a2 + a3 + a4 in x and y on the plane staged in P:  acc[e] += cx L_x + cy L_y  for the thread's cell.
-// Called by every thread of the block (it contains three block barriers).
+// Called by every thread of the block (it contains two block barriers).
 // ---------------------------------------------------------------------------------------------------------
 struct NoHook {
     __device__ __forceinline__ void operator()() const {}
@@ -223,13 +223,12 @@ __device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, cons
         for (int e = 0; e < NEQ; ++e) FxH[e * TY + i] = F[e];
         FxH[NEQ * TY + i] = uf;
     }
-    __syncthreads();                                                // S2: y right states have been read, rim fluxes are visible
-    if constexpr (D >= 2) {
+    if constexpr (D >= 2) {                                         // the fluxes have a buffer of their own: no barrier before this
 #pragma unroll
-        for (int e = 0; e < NEQ; ++e) B.X[e * NT + tid] = Fy[e];
+        for (int e = 0; e < NEQ; ++e) B.X2[e * NT + tid] = Fy[e];
         B.X8[tid] = ufy;
     }
-    __syncthreads();                                                // S3: fluxes are visible
+    __syncthreads();                                                // S2: fluxes (rim ones included) are visible
     if (i == 0) {
         const double du = B.ExF[NEQ * TY + j] - FxH[NEQ * TY + j];
 #pragma unroll
@@ -246,7 +245,7 @@ __device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, cons
         const double du = ufy - ufm;
 #pragma unroll
         for (int e = 0; e < NEQ; ++e) {
-            const double fm = j == 0 ? FyH[e * FTX + i] : B.X[e * NT + tid - FTX];
+            const double fm = j == 0 ? FyH[e * FTX + i] : B.X2[e * NT + tid - FTX];
             double rr = fm - Fy[e];
             if (e >= I::A) rr = fma(alpha_div_coef<NF>(eos, pc[e * PPL], pc[I::E * PPL]), du, rr);
             acc[e] = fma(cy, rr, acc[e]);
@@ -279,7 +278,7 @@ __global__ void __launch_bounds__(FTX *TY, 1)
     double *const rim = P + C::nP;
     double *const X8 = rim + C::nHx + C::nHy;
     double *const X = X8 + C::nX8;
-    const InplaneBufs<D, NF, TY> B(P, rim, X, X8);
+    const InplaneBufs<D, NF, TY> B(P, rim, X, X + NEQ * NT, X8);
 
     const int tid = threadIdx.x, i = tid & 31, j = tid >> 5;
     const int bx = blockIdx.x % ntx, by = blockIdx.x / ntx;
@@ -391,7 +390,8 @@ __global__ void __launch_bounds__(FTX *TY, 1)
     double *const rim = P + C::nP;
     double *const X8 = rim + C::nHx + C::nHy;
     double *const X = X8 + C::nX8;                                  // [NEQ][NT]    y exchange
-    double *const SQ = X + NEQ * NT;                                // [NEQ][NT]    raw q, own column, next plane
+    double *const X2 = X + NEQ * NT;                                // [NEQ][NT]    y exchange, fluxes
+    double *const SQ = X2 + NEQ * NT;                               // [NEQ][NT]    raw q, own column, next plane
     double *const SS = SQ + NEQ * NT;                               // [NEQ][NT]    raw q_s of the cell being written
     double *const SH = SS + NEQ * NT;                               // [2][NEQ][NH] raw q, halo cells of the next two staged planes
     unsigned *const tmem_word = reinterpret_cast<unsigned *>(SH + 2 * NEQ * NH);
@@ -542,7 +542,7 @@ __global__ void __launch_bounds__(FTX *TY, 1)
                 cp_async_wait<1>();
                 convert_staged(true, next_inplane ? ip + 1 : -1);
             };
-            const InplaneBufs<D, NF, TY> B(P, rim, X, X8);
+            const InplaneBufs<D, NF, TY> B(P, rim, X, X2, X8);
             inplane_xy<D, NF, TY, ORDER>(B, eos, cx, cy, acc, early, mid);
         } else {
             cp_async_wait<1>();
