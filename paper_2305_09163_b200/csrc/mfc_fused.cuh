@@ -11,17 +11,17 @@
 // planes ahead of the in-plane directions, so that when plane ip is differenced in x and y both of its z faces
 // are known by the end of the iteration and the cell is written once, complete.  Iteration m, ip = m - 3:
 //   * plane ip sits in P with a halo of 3 cells in x and y, laid out by the previous iteration: own cells from
-//     the ring of primitive planes, halo cells from raw q staged by cp.async two iterations earlier (ghost
+//     the ring of primitive planes (TMEM), halo cells from raw q staged by cp.async two iterations earlier (ghost
 //     cells take the wrapped / clamped interior cell);
 //   * x: each thread reconstructs its own cell from P; right states and fluxes move between neighbouring
-//     lanes by warp shuffles (tile width = warp width);  y: same, through shared memory (X = the ring slot
-//     plane ip left);  the rim of the tile (states of the cells just outside it, in x and in y) is
+//     lanes by warp shuffles (tile width = warp width);  y: same, through shared memory (right states and fluxes
+//     in a buffer each);  the rim of the tile (states of the cells just outside it, in x and in y) is
 //     reconstructed by the first four warps, the rim faces are solved by two warps;
 //   * while that runs, the raw column of plane m and the raw halo of plane ip + 1 (both landed) are converted
 //     to primitives in place (thread-private);
-//   * z: cell m - 2 is reconstructed from the thread-private window (plane m - 4 in registers, m - 3 in P,
-//     m - 2 and m - 1 in the ring, m just converted), face (m - 2) - 1/2 solved with the left state parked by
-//     the previous iteration and differenced against the previous flux (registers): the z part of cell ip;
+//   * z: cell m - 2 is reconstructed from the thread-private window (planes m - 4, m - 2, m - 1 in the TMEM
+//     scratch of the thread, m - 3 in P, m just converted), face (m - 2) - 1/2 solved with the left state parked
+//     by the previous iteration and differenced against the previous flux (both in TMEM): the z part of cell ip;
 //   * one store: out = ca q_n + cb q_s + coef (L_x + L_y + L_z); q_s staged by cp.async, q_n prefetched into L2;
 //   * "glue": P is restaged with plane ip + 1 and the raw reads of the next iterations are issued.  It has no
 //     FP64 work, so half of the warps of every scheduler run it before the z part and half after it.
@@ -29,7 +29,7 @@
 // barrier is involved in the staging, only cp.async.wait_group.
 // FP64 issue needs instruction-level parallelism rather than many warps on this part (one warp per scheduler
 // with four independent chains already reaches 92 % of the DFMA peak; weno5 x 7 + hllc alone run at 96 % with
-// 8 - 16 warps per SM), so a block is 8 - 12 warps with up to 168 - 255 registers each.  What the kernel loses
+// 8 - 16 warps per SM), so a block is 12 warps with up to 168 registers each.  What the kernel loses
 // against that figure is lost where all warps of a scheduler are in non-FP64 code at the same time.
 // 1D / 2D: one plane, no march: the same in-plane code on a directly loaded tile.
 #pragma once
@@ -318,7 +318,7 @@ __global__ void __launch_bounds__(FTX *TY, 1)
 // previous z flux and the plane that left the ring live there instead of in shared memory and registers.
 // A warp reaches the 32 TMEM lanes of its quarter (warp index mod 4), one lane per thread; the warps of a quarter
 // take disjoint column ranges.  tcgen05.ld / st with shape 32x32b move N consecutive 32-bit columns of the
-// thread's own lane to / from registers.  TV = values (doubles) per transfer: 8 (x16) or 16 (x32).
+// thread's own lane to / from registers.  TV = values (doubles) per slot: 8 (x16) or 10 (x16 + x4, three fluids).
 // ---------------------------------------------------------------------------------------------------------
 __device__ __forceinline__ void tmem_alloc512(unsigned *smem_word)
 {
@@ -332,20 +332,15 @@ __device__ __forceinline__ void tmem_dealloc512(unsigned base)
 template <int TV>
 __device__ __forceinline__ void tmem_load(unsigned a, double (&v)[TV])
 {
-    static_assert(TV == 8 || TV == 16, "8 or 16 doubles per transfer");
+    static_assert(TV == 8 || TV == 10, "8 doubles (x16) or 10 doubles (x16 + x4) per transfer");
     unsigned r[2 * TV];
-    if constexpr (TV == 8) {
-        asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
-                     : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
-                       "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
-                     : "r"(a));
-    } else {
-        asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
-                     : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
-                       "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]),
-                       "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]),
-                       "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
-                     : "r"(a));
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+                   "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+                 : "r"(a));
+    if constexpr (TV == 10) {
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];"
+                     : "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]) : "r"(a + 16u));
     }
     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #pragma unroll
@@ -357,18 +352,13 @@ __device__ __forceinline__ void tmem_store(unsigned a, const double (&v)[TV])
     unsigned r[2 * TV];
 #pragma unroll
     for (int k = 0; k < TV; ++k) { r[2 * k] = (unsigned)__double2loint(v[k]); r[2 * k + 1] = (unsigned)__double2hiint(v[k]); }
-    if constexpr (TV == 8) {
-        asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
-                     ::"r"(a), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]),
-                       "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
-                     : "memory");
-    } else {
-        asm volatile("tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31,%32};"
-                     ::"r"(a), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]),
-                       "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]), "r"(r[16]), "r"(r[17]),
-                       "r"(r[18]), "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]), "r"(r[24]), "r"(r[25]), "r"(r[26]),
-                       "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31])
-                     : "memory");
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
+                 ::"r"(a), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]),
+                   "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
+                 : "memory");
+    if constexpr (TV == 10) {
+        asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1,%2,%3,%4};"
+                     ::"r"(a + 16u), "r"(r[16]), "r"(r[17]), "r"(r[18]), "r"(r[19]) : "memory");
     }
     asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
 }
@@ -396,7 +386,7 @@ __global__ void __launch_bounds__(FTX *TY, 1)
     double *const SH = SS + NEQ * NT;                               // [2][NEQ][NH] raw q, halo cells of the next two staged planes
     unsigned *const tmem_word = reinterpret_cast<unsigned *>(SH + 2 * NEQ * NH);
     // thread-private TMEM scratch (see above): slots of TV doubles = 2 TV columns each
-    constexpr int TV = NEQ + 1 <= 8 ? 8 : 16;
+    constexpr int TV = NEQ + 1 <= 8 ? 8 : 10;
     enum { T_RING = 0, T_PARK = 4, T_PREV = 5, T_FLUX = 6, T_SLOTS = 7 };
     static_assert(T_SLOTS * 2 * TV * ((TY + 3) / 4) <= 512, "TMEM columns");
 

@@ -6,10 +6,10 @@
 #ifndef MFC_D
 #error "define MFC_D (1, 2 or 3) before including mfc_inst.cuh"
 #endif
-// rows of the 3D tile for up to two fluids (a multiple of 4: one warp per scheduler and group); -DMFC_TY_2F=8 builds
-// the 8-row variant measured in DESIGN.md 6.1
+// rows of the 3D tile (a multiple of 4: whole warps per scheduler); -DMFC_TY_2F=8 / 16 build the variants measured in
+// DESIGN.md 6.1
 #ifndef MFC_TY_2F
-#define MFC_TY_2F (NF <= 2 ? 12 : 8)
+#define MFC_TY_2F 12
 #endif
 #define MFC_CAT2(a, b) a##b
 #define MFC_CAT(a, b) MFC_CAT2(a, b)
@@ -40,8 +40,8 @@ cudaError_t MFC_CAT(launch_prim_d, MFC_D)(int nf, const Geo &g, const Eos &e, co
     return cudaGetLastError();
 }
 
-// tile height of the fused kernel: 3D tiles are sized so that the ring, the staging buffers and the staged plane
-// fit the 227 KB of one multiprocessor with 12 (two fluids) or 8 (three fluids) warps per block
+// tile height of the fused kernel: 3D tiles of 12 rows (12 warps, 168 registers per thread); the staged plane, the
+// exchange and staging buffers take 130 - 215 KB of shared memory, the z window of every column lives in TMEM
 template <int D, int NF>
 constexpr int fused_ty()
 {
