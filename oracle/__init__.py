@@ -37,25 +37,52 @@ class _Problem(C.Structure):
     ]
 
 
+STRICT_FLAGS = ["-O2", "-ffp-contract=off"]
+
+
+def _compile(target: Path, float_flags, force: bool = False) -> Path:
+    if force or not target.exists() or target.stat().st_mtime < _SRC.stat().st_mtime:
+        tmp = target.with_suffix(f".so.tmp{os.getpid()}")
+        cmd = ["gcc"] + list(float_flags) + ["-fopenmp", "-shared", "-fPIC", "-std=c99", str(_SRC), "-o", str(tmp), "-lm"]
+        subprocess.run(cmd, check=True)
+        os.replace(tmp, target)
+    return target
+
+
 def build(force: bool = False) -> Path:
     """Compile the oracle with gcc (-O2, no FMA contraction, OpenMP on the outer loops only)."""
-    if force or not _LIB.exists() or _LIB.stat().st_mtime < _SRC.stat().st_mtime:
-        tmp = _LIB.with_suffix(f".so.tmp{os.getpid()}")
-        cmd = ["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC", "-std=c99",
-               str(_SRC), "-o", str(tmp), "-lm"]
-        subprocess.run(cmd, check=True)
-        os.replace(tmp, _LIB)
-    return _LIB
+    return _compile(_LIB, STRICT_FLAGS, force)
 
 
-_lib = None
+def variant_flags():
+    """Floating-point flags of the SECOND build of the same source (tests/test_parity_norm.py): another correct
+    fp64 evaluation of the same formulas, used to measure how far two correct evaluations differ.  With FMA
+    hardware: contraction of every a*b+c (what nvcc does by default); without: reassociation and reciprocals."""
+    try:
+        with open("/proc/cpuinfo") as f:
+            has_fma = " fma " in f.read()
+    except OSError:
+        has_fma = False
+    if has_fma:
+        return ["-O2", "-ffp-contract=fast", "-mfma"], "fma"
+    return ["-O2", "-fassociative-math", "-fno-signed-zeros", "-fno-trapping-math", "-freciprocal-math"], "reassoc"
 
 
-def lib():
-    global _lib
-    if _lib is None:
-        build()
-        L = C.CDLL(str(_LIB))
+def build_variant(force: bool = False):
+    flags, tag = variant_flags()
+    return _compile(_HERE / f"libmfc_oracle_{tag}.so", flags, force), tag
+
+
+_libs = {}
+
+
+def lib(path: Path | None = None):
+    """The strict build (default) or, with `path`, another build of the same source (build_variant)."""
+    key = str(path) if path is not None else ""
+    if key not in _libs:
+        if path is None:
+            build()
+        L = C.CDLL(str(path if path is not None else _LIB))
         dp = C.POINTER(C.c_double)
         pp = C.POINTER(_Problem)
         L.orc_neq.argtypes = [pp]; L.orc_neq.restype = C.c_int
@@ -73,8 +100,8 @@ def lib():
         L.orc_kapila_K.argtypes = [pp, C.c_double, C.c_double]; L.orc_kapila_K.restype = C.c_double
         L.orc_threads.argtypes = []; L.orc_threads.restype = C.c_int
         L.orc_set_threads.argtypes = [C.c_int]; L.orc_set_threads.restype = None
-        _lib = L
-    return _lib
+        _libs[key] = L
+    return _libs[key]
 
 
 def _dp(a: np.ndarray):
@@ -85,8 +112,8 @@ def _dp(a: np.ndarray):
 class Oracle:
     """The oracle bound to one problem description."""
 
-    def __init__(self, prob):
-        self.L = lib()
+    def __init__(self, prob, lib_path: Path | None = None):
+        self.L = lib(lib_path)
         P = _Problem()
         P.ndim = int(prob.ndim)
         P.nf = len(prob.fluids)

@@ -19,7 +19,8 @@
  * independent), which changes no arithmetic.  Build: gcc -O2 -ffp-contract=off [-fopenmp] -shared -fPIC.
  *
  * Parity pins (tests/test_oracle_pins.py): every function below is pinned by something other than itself
- * (closed forms, exact Riemann solutions, polynomial exactness, invariants, numpy.pad).  The Davis
+ * (closed forms, exact Riemann solutions, polynomial exactness, invariants, numpy.pad; orc_line by differencing its
+ * fluxes into orc_rhs bit for bit; the mixture sound speed by a measured acoustic wave speed).  The Davis
  * wave-speed estimate and the u_face formula are pinned only through consistency/invariants (C2, C5, C7,
  * C8), not against MFC's own unpublished choice: "parity unpinned" w.r.t. MFC itself for those two readings.
  *

@@ -49,7 +49,7 @@ __device__ __forceinline__ double cell_signal_speed(const Geo &g, const Eos &eos
 #pragma unroll
     for (int e = 0; e < I::NA; ++e) { G = fma(wc[I::A + e], eos.dG[e], G); P = fma(wc[I::A + e], eos.dP[e], P); }
     const double num = fma(G, wc[I::E], P) + wc[I::E];               // (Gamma + 1) p + Pi
-    const double cs = num * rsqrt_fast(num * (G * rho));             // frozen mixture sound speed (reading B2)
+    const double cs = fabs(num) * rsqrt_fast(num * (G * rho));       // frozen mixture sound speed (reading B2)
     double s = 0.0;
 #pragma unroll
     for (int d = 0; d < D; ++d) s = fmax(s, g.inv_dx[d] * (fabs(wc[I::U + d]) + cs));

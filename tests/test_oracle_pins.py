@@ -688,3 +688,90 @@ def test_lower_order_uniform_state_and_conservation(order):
         line = np.ascontiguousarray(w[:, 0, 5, :])
         vL, vR, F, uf = orc.line(0, line)
         assert np.array_equal(vL[:, 1:-1], line[:, 3:-3]) and np.array_equal(vR[:, 1:-1], line[:, 3:-3])
+
+
+# ---------------------------------------------------------------------------------------------
+# orc_line (the checker of the GPU line tests): its face indexing is the one of orc_rhs
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("nf,periodic,order", [(1, True, 5), (2, False, 5), (3, True, 5), (2, True, 3), (2, False, 1)])
+def test_line_fluxes_differenced_reproduce_rhs_bitwise_in_1d(nf, periodic, order):
+    """Eq. 9-10 applied by hand to orc_line's F and u_face on a 1-D problem gives orc_rhs bit for bit:
+    F[:, j] is the flux of face j - 1/2 and F[:, j + 1] of face j + 1/2 of interior cell j, built from vL of cell j - 1 / j
+    and vR of cell j / j + 1.  Any slip of one in the face or state indexing of orc_line breaks it."""
+    import dataclasses
+    prob, q = wl.random_state(1, (57,), nf, seed=31 + nf, periodic=periodic)
+    prob = dataclasses.replace(prob, weno_order=order)
+    orc = oracle.Oracle(prob)
+    qf = q.copy()
+    L = orc.rhs(qf)[:, 0, 0, NG:-NG]                              # fills the ghosts of qf
+    w = np.ascontiguousarray(orc.cons_to_prim(qf)[:, 0, 0, :])    # [neq, n + 6]
+    vL, vR, F, uf = orc.line(0, w)
+    dx = prob.dx[0]
+    mine = (F[:, :-1] - F[:, 1:]) / dx
+    for i in range(nf - 1):
+        k = nf + 1 + 1 + i
+        mine[k] = mine[k] + qf[k, 0, 0, NG:-NG] * (uf[1:] - uf[:-1]) / dx
+    assert np.array_equal(mine, L)
+    # and the states themselves: vL[:, j + 1], vR[:, j + 1] belong to cell j (cells -1 .. n)
+    n = prob.n[0]
+    for e in range(prob.neq):
+        for j in (-1, 0, 7, n - 1, n):
+            s = w[e, NG + j - 2: NG + j + 3]
+            if order == 5:
+                l, r = oracle.weno5(*s, eps=prob.weno_eps)
+            elif order == 3:
+                l, r = oracle.weno3(*s[1:4], eps=prob.weno_eps)
+            else:
+                l = r = s[2]
+            assert vL[e, j + 1] == l and vR[e, j + 1] == r
+
+
+# ---------------------------------------------------------------------------------------------
+# Mixture sound speed away from the pure-fluid limit (reading B2): a MEASURED wave speed, not the formula
+# ---------------------------------------------------------------------------------------------
+def _acoustic_pulse_speed(alpha_w, p0, n=800):
+    """Speed at which a small pressure pulse splits and travels in a uniform two-fluid mixture at rest, measured from
+    the oracle's own time integration (a property of Eq. 6-10 + Eq. 1 with the mixture rule, whatever wave-speed
+    estimate the Riemann solver uses).  Returns (measured speed, problem, uniform conservative cell)."""
+    prob, _ = wl.random_state(1, (n,), 2, seed=1, periodic=True)
+    x = prob.centers(0)[None, None, :]
+    one = np.ones_like(x)
+    bump = np.exp(-((x - 0.5) / 0.03) ** 2)
+    q = wl.assemble(prob, [alpha_w * one, (1 - alpha_w) * one], [1000.0 * one, 50.0 * one], [0.0 * one], p0 * (1 + 1e-5 * bump))
+    q0 = wl.assemble(prob, [alpha_w * one, (1 - alpha_w) * one], [1000.0 * one, 50.0 * one], [0.0 * one], p0 * one)
+    orc = oracle.Oracle(prob)
+    t = 0.0
+    for _ in range(100000):
+        dt = orc.cfl_dt(q, 0.3)
+        orc.rk3_step(q, dt)
+        t += dt
+        dp = interior(prob, orc.cons_to_prim(q.copy()))[3, 0, 0] - p0
+        xs = prob.centers(0)
+        right = xs > 0.5
+        xr = np.sum(xs[right] * dp[right]) / np.sum(dp[right])
+        if xr > 0.8:
+            break
+    xl = np.sum(xs[~right] * dp[~right]) / np.sum(dp[~right])
+    return (xr - xl) / (2 * t), prob, q0, orc
+
+
+@pytest.mark.parametrize("alpha_w,p0", [(0.5, 5.0e8), (0.3, 1.0e5), (0.9, 2.0e9)])
+def test_mixture_sound_speed_is_the_measured_acoustic_speed(alpha_w, p0):
+    """(i) The speed c that orc_cfl_dt uses (dt = cfl dx / c for a fluid at rest) is the speed at which a small
+    pressure pulse actually travels in the alpha_water = 0.5 (0.3, 0.9) mixture: they agree to 2e-5 (measured 1470.85,
+    615.42, 2829.10 m/s), asserted to 1e-3.  At these states Wood's (equilibrium) speed is off by +3.8 %, -96 %, +9.9 %,
+    the volume-weighted average of the pure-fluid speeds by +102 %, -15 %, +34 %, and Gamma p + Pi without the "+ p" by
+    -17 %, -0.02 %, -32 %: each plausible mistake fails at least two of the three.  (ii) orc_hllc uses the same
+    speed: with u_L = u_R = u and different pressures the flux is exactly F(q_L) (Eq. 13-14, supersonic branch:
+    s_L = min(u - c_L, u - c_R) > 0) for u = 1.01 c and depends on the right state for u = 0.99 c."""
+    c_meas, prob, q0, orc = _acoustic_pulse_speed(alpha_w, p0)
+    c_cfl = prob.dx[0] / orc.cfl_dt(q0, 1.0)
+    assert abs(c_cfl / c_meas - 1.0) < 1e-3, (c_cfl, c_meas)
+    w = orc.cons_to_prim_cell(q0[:, 0, 0, NG])
+    for factor, supersonic in [(1.01, True), (0.99, False)]:
+        wl_, wr_ = w.copy(), w.copy()
+        wl_[2] = wr_[2] = factor * c_meas
+        wr_[3] = w[3] * (1 - 1e-6)                                # c_R barely changes; the flux would see p_R if subsonic
+        F, uf = orc.hllc(0, wl_, wr_)
+        Fsame, _ = orc.hllc(0, wl_, wl_)                          # = F(q_L) by consistency (C2)
+        assert np.array_equal(F, Fsame) == supersonic
