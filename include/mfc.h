@@ -18,9 +18,14 @@
  *   given to mfc_init; names ending in _host are HOST pointers.  The caller owns every buffer it passes;
  *   the library owns its scratch (two Runge-Kutta stage arrays, reduction workspace), allocated in mfc_init
  *   and released in mfc_destroy.
- * Boundary conditions are applied while a tile of the state is staged on chip (a ghost cell is computed from
- *   the wrapped / clamped interior cell).  Ghost cells of q are therefore never read and never
- *   written; ghost entries of rhs are unspecified.
+ * Boundary conditions: every evaluation of L first fills the ghost cells of its input array in memory
+ *   (periodic wrap / zero-gradient copy of the nearest interior cell, corners included).  The ghost cells of q are
+ *   therefore OVERWRITTEN by mfc_rhs and mfc_rk3_step (as SURVEY.md 8(b) specifies); their previous contents are never
+ *   read.  Ghost entries of rhs are unspecified.
+ * Tensor memory: the 3D kernel keeps its z window in tensor memory and allocates ALL 512 TMEM columns of every
+ *   multiprocessor for as long as one of its blocks is resident (one block per multiprocessor).  A kernel of another
+ *   stream or process that allocates tensor memory on the same device (any tcgen05 GEMM, e.g. a bf16 matmul) is
+ *   serialised against it by the hardware allocator: it waits, results are unaffected.
  * Streams: `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  All work is
  *   enqueued on it.  Only mfc_cfl_dt, mfc_advance_host, mfc_profile_get and mfc_probe_dfma synchronise.
  * Errors: every function returns MFC_OK (0) or a negative mfc_status; nothing is thrown or printed.
@@ -75,6 +80,10 @@ typedef struct {
     int kapila;        /* != 0: Kapila model, the alpha row carries the source K div(u) with the two-fluid K of Eq. 2
                           (PAPER.md:52, 60-62), cell-centred, on the same face-velocity differences as alpha div(u);
                           needs n_fluids == 2 and volume fractions inside (0, 1).  0: Allaire model, K = 0 */
+    int staging;       /* how the 3D kernel stages its tiles: 0 = TMA boxes (cp.async.bulk.tensor) where the layout allows
+                          them -- even padded extent in x (n[0] even) and a 16-byte aligned q_dev -- else per-thread
+                          cp.async; 1 = TMA only (calls fail with MFC_ECUDA where it does not apply); 2 = cp.async only.
+                          Both paths compute the same bits */
 } mfc_opts;
 
 typedef struct mfc_ctx mfc_ctx;
@@ -94,11 +103,13 @@ int mfc_layout(const mfc_ctx *ctx, int *neq, int *ng, long long padded_n[3], lon
  *   cons->prim with ghost fill -> per direction WENO5-JS (Eq. 12,
  *   Listing 1) -> HLLC flux and face velocity (Eq. 13-14) ->
  *   rhs_k = sum_d (F_{k,-1/2} - F_{k,+1/2})/dx_d  [+ (alpha_i + K) sum_d (u_{+1/2} - u_{-1/2})/dx_d on alpha rows].
- * q_dev is read (interior only); the interior of rhs_dev is written.  q_dev and rhs_dev must not alias. */
-int mfc_rhs(mfc_ctx *ctx, const double *q_dev, double *rhs_dev, void *stream);
+ * The ghost cells of q_dev are overwritten with the boundary fill, its interior is read; the interior of rhs_dev is
+ * written.  q_dev and rhs_dev must not alias. */
+int mfc_rhs(mfc_ctx *ctx, double *q_dev, double *rhs_dev, void *stream);
 
 /* One 3-stage TVD Runge-Kutta step of size dt, in place on the interior of q_dev (ref. [19]):
- *   q1 = q + dt L(q);  q2 = 3/4 q + 1/4 (q1 + dt L(q1));  q <- 1/3 q + 2/3 (q2 + dt L(q2)). */
+ *   q1 = q + dt L(q);  q2 = 3/4 q + 1/4 (q1 + dt L(q1));  q <- 1/3 q + 2/3 (q2 + dt L(q2)).
+ * On return the ghost cells of q_dev hold the boundary fill of the state the step STARTED from. */
 int mfc_rk3_step(mfc_ctx *ctx, double *q_dev, double dt, void *stream);
 
 /* CFL-restricted time step: dt = cfl * min over interior cells and directions of
@@ -130,7 +141,8 @@ typedef enum {
                        flux difference and RK stage combine in one launch */
     MFC_K_CFL = 1,  /* CFL reduction */
     MFC_K_PRIM = 2, /* stage output of mfc_cons_to_prim (parity tests only; not on the path) */
-    MFC_K_COUNT = 3
+    MFC_K_GHOST = 3, /* ghost fill in memory, once before every evaluation of L */
+    MFC_K_COUNT = 4
 } mfc_kernel_id;
 
 /* With profiling on, every kernel launch is bracketed by CUDA events on its own stream. */
@@ -146,6 +158,8 @@ long long mfc_launch_count(const mfc_ctx *ctx);
 int mfc_probe_dfma(int device, double *tflops_host, double *ms_host);
 
 const char *mfc_strerror(int code);
+/* Text of the CUDA runtime error behind the last MFC_ECUDA / MFC_ENOMEM a kernel launch of this context returned. */
+const char *mfc_cuda_error(const mfc_ctx *ctx);
 const char *mfc_version(void);
 
 #ifdef __cplusplus

@@ -16,14 +16,15 @@ LIB_PATH = _HERE / "libmfc_b200.so"
 MFC_NG = 3
 MFC_OK, MFC_EINVAL, MFC_EUNSUPPORTED, MFC_ECUDA, MFC_ENOMEM = 0, -1, -2, -3, -4
 MFC_BC_PERIODIC, MFC_BC_EXTRAP = 0, 1
-MFC_K_RHS, MFC_K_CFL, MFC_K_PRIM, MFC_K_COUNT = 0, 1, 2, 3
-KERNEL_NAMES = {MFC_K_RHS: "rhs_fused", MFC_K_CFL: "cfl", MFC_K_PRIM: "prim"}
+MFC_K_RHS, MFC_K_CFL, MFC_K_PRIM, MFC_K_GHOST, MFC_K_COUNT = 0, 1, 2, 3, 4
+KERNEL_NAMES = {MFC_K_RHS: "rhs_fused", MFC_K_CFL: "cfl", MFC_K_PRIM: "prim", MFC_K_GHOST: "ghost_fill"}
+MFC_STAGING_AUTO, MFC_STAGING_TMA, MFC_STAGING_CPASYNC = 0, 1, 2
 
 # every symbol include/mfc.h declares
 EXPORTS = [
     "mfc_init", "mfc_destroy", "mfc_layout", "mfc_rhs", "mfc_rk3_step", "mfc_cfl_dt", "mfc_advance_host",
     "mfc_cons_to_prim", "mfc_line_fluxes", "mfc_profile_enable", "mfc_profile_get", "mfc_launch_count",
-    "mfc_probe_dfma", "mfc_strerror", "mfc_version",
+    "mfc_probe_dfma", "mfc_strerror", "mfc_version", "mfc_cuda_error",
 ]
 
 
@@ -51,7 +52,7 @@ class mfc_bc(C.Structure):
 
 class mfc_opts(C.Structure):
     _fields_ = [("weno_eps", C.c_double), ("cfl", C.c_double), ("device", C.c_int), ("march_segment", C.c_int),
-                ("weno_order", C.c_int), ("kapila", C.c_int)]
+                ("weno_order", C.c_int), ("kapila", C.c_int), ("staging", C.c_int)]
 
 
 _lib = None
@@ -87,6 +88,7 @@ def lib():
     L.mfc_probe_dfma.argtypes = [C.c_int, dp, dp]; L.mfc_probe_dfma.restype = C.c_int
     L.mfc_strerror.argtypes = [C.c_int]; L.mfc_strerror.restype = C.c_char_p
     L.mfc_version.argtypes = []; L.mfc_version.restype = C.c_char_p
+    L.mfc_cuda_error.argtypes = [vp]; L.mfc_cuda_error.restype = C.c_char_p
     _lib = L
     return L
 
@@ -105,7 +107,7 @@ def mfc_version() -> str:
 
 
 def mfc_init(grid_n, lo, hi, fluids, bc_lo, bc_hi, *, weno_eps=1e-16, cfl=0.3, device=-1, march_segment=0, weno_order=5,
-             kapila=False):
+             kapila=False, staging=MFC_STAGING_AUTO):
     """grid_n / lo / hi: one entry per active dimension; fluids: [(gamma, pi_inf), ...]; returns the context handle."""
     ndim = len(grid_n)
     g = mfc_grid()
@@ -120,7 +122,8 @@ def mfc_init(grid_n, lo, hi, fluids, bc_lo, bc_hi, *, weno_eps=1e-16, cfl=0.3, d
     fl = (mfc_fluid * max(1, len(fluids)))()
     for i, (gam, pinf) in enumerate(fluids):
         fl[i].gamma, fl[i].pi_inf = float(gam), float(pinf)
-    o = mfc_opts(float(weno_eps), float(cfl), int(device), int(march_segment), int(weno_order), 1 if kapila else 0)
+    o = mfc_opts(float(weno_eps), float(cfl), int(device), int(march_segment), int(weno_order), 1 if kapila else 0,
+                 int(staging))
     h = C.c_void_p()
     _check(lib().mfc_init(C.byref(h), C.byref(g), len(fluids), fl, C.byref(b), C.byref(o)), "mfc_init")
     return h
@@ -138,12 +141,22 @@ def mfc_layout(ctx):
     return neq.value, ng.value, (pn[0], pn[1], pn[2]), el.value
 
 
+def mfc_cuda_error(ctx) -> str:
+    return lib().mfc_cuda_error(ctx).decode()
+
+
+def _check_ctx(code: int, where: str, ctx) -> None:
+    if code in (MFC_ECUDA, MFC_ENOMEM):
+        raise MfcError(code, f"{where} [{mfc_cuda_error(ctx)}]")
+    _check(code, where)
+
+
 def mfc_rhs(ctx, q_dev: int, rhs_dev: int, stream: int = 0) -> None:
-    _check(lib().mfc_rhs(ctx, q_dev, rhs_dev, stream), "mfc_rhs")
+    _check_ctx(lib().mfc_rhs(ctx, q_dev, rhs_dev, stream), "mfc_rhs", ctx)
 
 
 def mfc_rk3_step(ctx, q_dev: int, dt: float, stream: int = 0) -> None:
-    _check(lib().mfc_rk3_step(ctx, q_dev, float(dt), stream), "mfc_rk3_step")
+    _check_ctx(lib().mfc_rk3_step(ctx, q_dev, float(dt), stream), "mfc_rk3_step", ctx)
 
 
 def mfc_cfl_dt(ctx, q_dev: int, stream: int = 0) -> float:

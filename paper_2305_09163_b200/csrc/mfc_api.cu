@@ -23,12 +23,12 @@ cudaError_t launch_prim(int ndim, int nf, const Geo &g, const Eos &e, const doub
     return cudaErrorInvalidValue;
 }
 cudaError_t launch_rhs(int ndim, int nf, int order, const Geo &g, const Eos &e, const double *q, const SweepOut &o, int segment,
-                       cudaStream_t s)
+                       int path, cudaStream_t s)
 {
     switch (ndim) {
-        case 1: return launch_rhs_d1(nf, order, g, e, q, o, segment, s);
-        case 2: return launch_rhs_d2(nf, order, g, e, q, o, segment, s);
-        case 3: return launch_rhs_d3(nf, order, g, e, q, o, segment, s);
+        case 1: return launch_rhs_d1(nf, order, g, e, q, o, segment, path, s);
+        case 2: return launch_rhs_d2(nf, order, g, e, q, o, segment, path, s);
+        case 3: return launch_rhs_d3(nf, order, g, e, q, o, segment, path, s);
     }
     return cudaErrorInvalidValue;
 }
@@ -51,6 +51,58 @@ cudaError_t launch_line(int ndim, int nf, int order, int dir, const Eos &e, int 
         case 3: return launch_line_d3(nf, order, dir, e, n, w, vL, vR, F, uf, s);
     }
     return cudaErrorInvalidValue;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// a0 ghost fill in memory ("buffers at the domain edges"): every ghost cell of the padded box takes the
+// wrapped (periodic) or clamped (extrapolation) interior cell, dimension by dimension -- the index map composes, so
+// one pass gives what filling x, then y, then z over the full padded extents gives, corners included.  Run before
+// every evaluation of L: the TMA-staged march kernel then reads plain boxes of the padded array (a tile's halo is
+// just the neighbouring cells, whatever the boundary kind).  One thread per ghost cell; the ghost shell is enumerated
+// as the z slabs (full planes), the y slabs (full rows of the interior planes) and the x slabs (the rest).
+// ---------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) ghost_fill_kernel(Geo g, int neq, double *q)
+{
+    const long long nzs = (long long)(g.p[2] - g.n[2]) * g.p[1] * g.p[0];           // z slabs: 2 g[2] planes
+    const long long nys = (long long)g.n[2] * (g.p[1] - g.n[1]) * g.p[0];           // y slabs: 2 g[1] rows per interior plane
+    const long long nxs = (long long)g.n[2] * g.n[1] * (g.p[0] - g.n[0]);           // x slabs: 2 g[0] cells per interior row
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    int i, j, k;
+    if (t < nzs) {
+        i = (int)(t % g.p[0]);
+        const long long r = t / g.p[0];
+        j = (int)(r % g.p[1]);
+        const int kk = (int)(r / g.p[1]);
+        k = kk < g.g[2] ? kk : kk + g.n[2];
+    } else if (t < nzs + nys) {
+        const long long u = t - nzs;
+        i = (int)(u % g.p[0]);
+        const long long r = u / g.p[0];
+        const int jj = (int)(r % (2 * g.g[1]));
+        j = jj < g.g[1] ? jj : jj + g.n[1];
+        k = (int)(r / (2 * g.g[1])) + g.g[2];
+    } else if (t < nzs + nys + nxs) {
+        const long long u = t - nzs - nys;
+        const int ii = (int)(u % (2 * g.g[0]));
+        i = ii < g.g[0] ? ii : ii + g.n[0];
+        const long long r = u / (2 * g.g[0]);
+        j = (int)(r % g.n[1]) + g.g[1];
+        k = (int)(r / g.n[1]) + g.g[2];
+    } else return;
+    const int si = bc_source(i - g.g[0], g.n[0], g.bc_lo[0], g.bc_hi[0]) + g.g[0];
+    const int sj = bc_source(j - g.g[1], g.n[1], g.bc_lo[1], g.bc_hi[1]) + g.g[1];
+    const int sk = bc_source(k - g.g[2], g.n[2], g.bc_lo[2], g.bc_hi[2]) + g.g[2];
+    const long long dst = (long long)k * g.sz + (long long)j * g.sy + i;
+    const long long src = (long long)sk * g.sz + (long long)sj * g.sy + si;
+    for (int e = 0; e < neq; ++e) q[(long long)e * g.cells + dst] = q[(long long)e * g.cells + src];
+}
+
+cudaError_t launch_ghost_fill(const Geo &g, int neq, double *q, cudaStream_t s)
+{
+    const long long shell = g.cells - (long long)g.n[0] * g.n[1] * g.n[2];
+    if (shell <= 0) return cudaSuccess;
+    ghost_fill_kernel<<<(unsigned)((shell + 255) / 256), 256, 0, s>>>(g, neq, q);
+    return cudaGetLastError();
 }
 
 __global__ void eos_seed_kernel(const double *gm1, double *ygm1, int n)
@@ -84,7 +136,7 @@ struct EventPair {
 }  // namespace mfc
 
 struct mfc_ctx {
-    int ndim = 0, nf = 0, neq = 0, device = 0, segment = 0, order = 5;
+    int ndim = 0, nf = 0, neq = 0, device = 0, segment = 0, order = 5, staging = 0;
     double cfl = 0.3;
     long long elems = 0;
     mfc::Geo g{};
@@ -95,9 +147,10 @@ struct mfc_ctx {
     bool profile = false;
     std::vector<mfc::EventPair> pending;
     std::vector<cudaEvent_t> pool;
-    double ms[MFC_K_COUNT] = {0, 0, 0};
-    long long launches[MFC_K_COUNT] = {0, 0, 0};
+    double ms[MFC_K_COUNT] = {0, 0, 0, 0};
+    long long launches[MFC_K_COUNT] = {0, 0, 0, 0};
     long long launch_total = 0;
+    cudaError_t last_cuda = cudaSuccess;     // the CUDA error behind the last MFC_ECUDA / MFC_ENOMEM of this context
 };
 
 namespace {
@@ -156,22 +209,29 @@ struct Timed {
     }
 };
 
-int cuda_to_status(cudaError_t e)
+int cuda_to_status(cudaError_t e, mfc_ctx *c = nullptr)
 {
     if (e == cudaSuccess) return MFC_OK;
+    if (c) c->last_cuda = e;
     if (e == cudaErrorMemoryAllocation) return MFC_ENOMEM;
     return MFC_ECUDA;
 }
 
-// One evaluation of L(q_in), one launch: out = base + coef L(q_in), base described by `o` (SweepOut, mfc_launch.h).
-int eval_L(mfc_ctx *c, const double *q_in, const SweepOut &o, cudaStream_t s)
+// One evaluation of L(q_in): the ghost cells of q_in are filled in memory (a0), then one launch computes
+// out = base + coef L(q_in), base described by `o` (SweepOut, mfc_launch.h).
+int eval_L(mfc_ctx *c, double *q_in, const SweepOut &o, cudaStream_t s)
 {
     cudaError_t err;
     {
-        Timed t(c, MFC_K_RHS, s);
-        err = launch_rhs(c->ndim, c->nf, c->order, c->g, c->e, q_in, o, c->segment, s);
+        Timed t(c, MFC_K_GHOST, s);
+        err = launch_ghost_fill(c->g, c->neq, q_in, s);
     }
-    return cuda_to_status(err);
+    if (err != cudaSuccess) return cuda_to_status(err, c);
+    {
+        Timed t(c, MFC_K_RHS, s);
+        err = launch_rhs(c->ndim, c->nf, c->order, c->g, c->e, q_in, o, c->segment, c->staging, s);
+    }
+    return cuda_to_status(err, c);
 }
 
 // 3-stage TVD Runge-Kutta.  Every stage is out = ca qn + cb (qs + dt L(qs)).  A stage reads its
@@ -239,7 +299,9 @@ const char *mfc_strerror(int code)
     return "unknown error";
 }
 
-const char *mfc_version(void) { return "mfc-b200 0.1 (sm_100a)"; }
+const char *mfc_version(void) { return "mfc-b200 0.2 (sm_100a)"; }
+
+const char *mfc_cuda_error(const mfc_ctx *c) { return c ? cudaGetErrorString(c->last_cuda) : "no context"; }
 
 int mfc_init(mfc_ctx **out, const mfc_grid *grid, int n_fluids, const mfc_fluid *eos, const mfc_bc *bc, const mfc_opts *opts)
 {
@@ -250,6 +312,7 @@ int mfc_init(mfc_ctx **out, const mfc_grid *grid, int n_fluids, const mfc_fluid 
     if (opts && opts->kapila && n_fluids != 2) return MFC_EUNSUPPORTED;
     const int order = (opts && opts->weno_order != 0) ? opts->weno_order : 5;
     if (order != 1 && order != 3 && order != 5) return MFC_EINVAL;
+    if (opts && (opts->staging < 0 || opts->staging > 2)) return MFC_EINVAL;
     for (int d = 0; d < grid->ndim; ++d) {
         if (grid->n[d] < MFC_NG || !(grid->hi[d] > grid->lo[d])) return MFC_EINVAL;
         if (bc->lo[d] != MFC_BC_PERIODIC && bc->lo[d] != MFC_BC_EXTRAP) return MFC_EINVAL;
@@ -311,6 +374,7 @@ int mfc_init(mfc_ctx **out, const mfc_grid *grid, int n_fluids, const mfc_fluid 
     e.kapila = (opts && opts->kapila) ? 1 : 0;
 
     c->segment = (opts && opts->march_segment > 0) ? opts->march_segment : 0;   // 0: the launcher's heuristic
+    c->staging = opts ? opts->staging : 0;
 
     DeviceGuard guard(dev);
     if (cudaDeviceGetAttribute(&g.sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) g.sms = 0;
@@ -364,7 +428,7 @@ int mfc_layout(const mfc_ctx *c, int *neq, int *ng, long long padded_n[3], long 
     return MFC_OK;
 }
 
-int mfc_rhs(mfc_ctx *c, const double *q_dev, double *rhs_dev, void *stream)
+int mfc_rhs(mfc_ctx *c, double *q_dev, double *rhs_dev, void *stream)
 {
     if (!c || !q_dev || !rhs_dev || q_dev == rhs_dev) return MFC_EINVAL;
     DeviceGuard guard(c->device);

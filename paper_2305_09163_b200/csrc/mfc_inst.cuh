@@ -2,6 +2,7 @@
 // NF in {1,2,3}.  One translation unit per D keeps the sm_100a compile parallel.
 #include "mfc_kernels.cuh"
 #include "mfc_fused.cuh"
+#include "mfc_fused_tma.cuh"
 
 #ifndef MFC_D
 #error "define MFC_D (1, 2 or 3) before including mfc_inst.cuh"
@@ -69,39 +70,88 @@ static int fused_segment(const Geo &g, long long tiles, int wanted)
     return best_seg;
 }
 
+// The opt-in to more than 48 KB of dynamic shared memory is a property of the kernel, not of the launch: set once per
+// instantiation and process (a function-local static of launch_fused<D, NF, ORDER>), and its status kept: a failed
+// opt-in is reported by every later launch
+#define MFC_OPTIN_SHARED(kernel, bytes)                                                                               \
+    [&]() -> cudaError_t {                                                                                            \
+        static const cudaError_t st_ = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes); \
+        return st_;                                                                                                   \
+    }()
+
+// rank-4 tensor map (x, y, z, equation) of the padded state array with a box of bx x by cells of one plane, all equations
+static bool encode_state_map(CUtensorMap *map, const Geo &g, int neq, const double *base, int bx, int by)
+{
+    typedef CUresult (*encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                  const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static encode_fn fn = []() -> encode_fn {
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qr) != cudaSuccess || qr != cudaDriverEntryPointSuccess)
+            return nullptr;
+        return reinterpret_cast<encode_fn>(p);
+    }();
+    if (!fn) return false;
+    const cuuint64_t dims[4] = {(cuuint64_t)g.p[0], (cuuint64_t)g.p[1], (cuuint64_t)g.p[2], (cuuint64_t)neq};
+    const cuuint64_t strides[3] = {(cuuint64_t)g.sy * 8, (cuuint64_t)g.sz * 8, (cuuint64_t)g.cells * 8};
+    const cuuint32_t box[4] = {(cuuint32_t)bx, (cuuint32_t)by, 1, (cuuint32_t)neq};
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    return fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<double *>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+              CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 template <int D, int NF, int ORDER>
-static void launch_fused(const Geo &g, const Eos &e, const double *q, const SweepOut &o, int segment, cudaStream_t s)
+static cudaError_t launch_fused(const Geo &g, const Eos &e, const double *q, const SweepOut &o, int segment, int path, cudaStream_t s)
 {
     constexpr int TY = fused_ty<D, NF>();
     using C = FusedCfg<D, NF, TY>;
     static_assert(C::bytes <= 227 * 1024, "fused tile does not fit shared memory");
     const int ntx = (g.n[0] + FTX - 1) / FTX;
     const int nty = D >= 2 ? (g.n[1] + TY - 1) / TY : 1;
+    cudaError_t st;
     if constexpr (D == 3) {
+        // one block per multiprocessor is what the TMEM allocation (all 512 columns) relies on
+        static_assert(2 * C::bytes > 227 * 1024, "two resident blocks would deadlock in tcgen05.alloc");
         const int seg = fused_segment(g, (long long)ntx * nty, segment);
         const int nseg = (g.n[2] + seg - 1) / seg;
-        cudaFuncSetAttribute(rhs_fused_march_kernel<NF, TY, ORDER>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::bytes);
-        rhs_fused_march_kernel<NF, TY, ORDER><<<(unsigned)((long long)ntx * nty * nseg), C::NT, C::bytes, s>>>(g, e, q, o, ntx, nty, seg);
+        const unsigned blocks = (unsigned)((long long)ntx * nty * nseg);
+        // TMA staging needs 16-byte aligned rows (even padded extent, aligned base) and q_s = the array L is evaluated on
+        using T = TmaCfg<NF, TY>;
+        static_assert(T::bytes <= 227 * 1024, "TMA-staged tile does not fit shared memory");
+        const bool tma_ok = path != MFC_PATH_LDGSTS && (g.p[0] & 1) == 0 && (reinterpret_cast<unsigned long long>(q) & 15) == 0 &&
+                            (o.nbase == 0 || o.qs == q);
+        CUtensorMap tm_plane, tm_col;
+        if (tma_ok && encode_state_map(&tm_plane, g, C::NEQ, q, FPX, C::PY) && encode_state_map(&tm_col, g, C::NEQ, q, T::CW, TY)) {
+            if ((st = MFC_OPTIN_SHARED((rhs_fused_march_tma_kernel<NF, TY, ORDER>), T::bytes)) != cudaSuccess) return st;
+            rhs_fused_march_tma_kernel<NF, TY, ORDER><<<blocks, C::NT, T::bytes, s>>>(tm_plane, tm_col, g, e, o, ntx, nty, seg);
+        } else {
+            if (path == MFC_PATH_TMA) return cudaErrorInvalidValue;
+            if ((st = MFC_OPTIN_SHARED((rhs_fused_march_kernel<NF, TY, ORDER>), C::bytes)) != cudaSuccess) return st;
+            rhs_fused_march_kernel<NF, TY, ORDER><<<blocks, C::NT, C::bytes, s>>>(g, e, q, o, ntx, nty, seg);
+        }
     } else {
-        cudaFuncSetAttribute(rhs_fused_plane_kernel<D, NF, TY, ORDER>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::bytes);
+        if ((st = MFC_OPTIN_SHARED((rhs_fused_plane_kernel<D, NF, TY, ORDER>), C::bytes)) != cudaSuccess) return st;
         rhs_fused_plane_kernel<D, NF, TY, ORDER><<<(unsigned)((long long)ntx * nty), C::NT, C::bytes, s>>>(g, e, q, o, ntx);
     }
-}
-
-template <int D, int NF>
-static cudaError_t launch_fused_order(int order, const Geo &g, const Eos &e, const double *q, const SweepOut &o, int segment,
-                                      cudaStream_t s)
-{
-    MFC_FOR_ORDER(order, (launch_fused<D, NF, ORDER>(g, e, q, o, segment, s)))
     return cudaSuccess;
 }
 
+template <int D, int NF>
+static cudaError_t launch_fused_order(int order, const Geo &g, const Eos &e, const double *q, const SweepOut &o, int segment, int path,
+                                      cudaStream_t s)
+{
+    cudaError_t st = cudaSuccess;
+    MFC_FOR_ORDER(order, (st = launch_fused<D, NF, ORDER>(g, e, q, o, segment, path, s)))
+    return st;
+}
+
 cudaError_t MFC_CAT(launch_rhs_d, MFC_D)(int nf, int order, const Geo &g, const Eos &e, const double *q, const SweepOut &o,
-                                         int segment, cudaStream_t s)
+                                         int segment, int path, cudaStream_t s)
 {
     constexpr int D = MFC_D;
     cudaError_t err = cudaSuccess;
-    MFC_FOR_NF(nf, (err = launch_fused_order<D, NF>(order, g, e, q, o, segment, s)))
+    MFC_FOR_NF(nf, (err = launch_fused_order<D, NF>(order, g, e, q, o, segment, path, s)))
     return err != cudaSuccess ? err : cudaGetLastError();
 }
 

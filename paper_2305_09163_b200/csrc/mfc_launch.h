@@ -48,8 +48,12 @@ struct SweepOut {
 };
 
 cudaError_t launch_prim(int ndim, int nf, const Geo &g, const Eos &e, const double *q, double *w, cudaStream_t s);
+// staging path of the 3D kernel: AUTO = TMA boxes where the layout allows them (even padded extent in x, 16-byte
+// aligned base), else per-thread cp.async; the other two force one of them (TMA fails if the layout does not allow it)
+enum { MFC_PATH_AUTO = 0, MFC_PATH_TMA = 1, MFC_PATH_LDGSTS = 2 };
 cudaError_t launch_rhs(int ndim, int nf, int order, const Geo &g, const Eos &e, const double *q, const SweepOut &o, int segment,
-                       cudaStream_t s);
+                       int path, cudaStream_t s);
+cudaError_t launch_ghost_fill(const Geo &g, int neq, double *q, cudaStream_t s);
 cudaError_t launch_cfl(int ndim, int nf, const Geo &g, const Eos &e, const double *q, unsigned long long *min_bits,
                        cudaStream_t s);
 cudaError_t launch_eos_seed(const double *gm1_dev, double *ygm1_dev, int n, cudaStream_t s);
@@ -60,7 +64,7 @@ cudaError_t launch_line(int ndim, int nf, int order, int dir, const Eos &e, int 
 #define MFC_DECL_DIM(D)                                                                                               \
     cudaError_t launch_prim_d##D(int nf, const Geo &g, const Eos &e, const double *q, double *w, cudaStream_t s);     \
     cudaError_t launch_rhs_d##D(int nf, int order, const Geo &g, const Eos &e, const double *q, const SweepOut &o, int segment,  \
-                                cudaStream_t s);                                                                      \
+                                int path, cudaStream_t s);                                                            \
     cudaError_t launch_cfl_d##D(int nf, const Geo &g, const Eos &e, const double *q, unsigned long long *min_bits,    \
                                 cudaStream_t s);                                                                      \
     cudaError_t launch_line_d##D(int nf, int order, int dir, const Eos &e, int n, const double *w, double *vL, double *vR,       \

@@ -78,19 +78,28 @@ def test_prim_mixed_boundary_kinds():
     assert np.array_equal(got, ref)
 
 
-def test_ghost_cells_of_q_are_not_touched():
-    prob, q = wl.random_state(2, (12, 9), 2, seed=8, periodic=True)
-    q[...] = np.where(q == 0.0, 12345.0, q)  # mark the ghosts
+@pytest.mark.parametrize("ndim,n,lo,hi", [
+    (1, (37,), (wl.BC_EXTRAP,), (wl.BC_EXTRAP,)), (2, (12, 9), (wl.BC_PERIODIC, wl.BC_EXTRAP), (wl.BC_PERIODIC, wl.BC_EXTRAP)),
+    (3, (10, 7, 5), (wl.BC_PERIODIC,) * 3, (wl.BC_PERIODIC,) * 3),
+    (3, (9, 8, 6), (wl.BC_EXTRAP, wl.BC_PERIODIC, wl.BC_EXTRAP), (wl.BC_EXTRAP, wl.BC_PERIODIC, wl.BC_EXTRAP))])
+def test_ghost_cells_of_q_hold_the_boundary_fill_after_rhs(ndim, n, lo, hi):
+    """a0 in memory ("ghost cells of q are overwritten by every mfc_rhs"): whatever the ghost
+    cells held, after mfc_rhs the whole padded array equals the oracle's ghost fill, corners included, bit for bit."""
+    import dataclasses
+    prob, q = wl.random_state(ndim, n, 2, seed=8, periodic=True)
+    prob = dataclasses.replace(prob, bc_lo=tuple(lo) + (wl.BC_EXTRAP,) * (3 - ndim), bc_hi=tuple(hi) + (wl.BC_EXTRAP,) * (3 - ndim))
+    core = q[prob.interior()].copy()
+    q[...] = np.random.default_rng(0).normal(size=q.shape)  # garbage in the ghosts
+    q[prob.interior()] = core
+    ref = q.copy()
+    oracle.Oracle(prob).fill_ghosts(ref)
     with Gpu(prob) as g:
         qd = g.to_dev(q)
         out = g.torch.zeros_like(qd)
         B.mfc_rhs(g.ctx, qd.data_ptr(), out.data_ptr(), g.stream)
-        B.mfc_rk3_step(g.ctx, qd.data_ptr(), 1e-9, g.stream)
         g.torch.cuda.synchronize()
         after = qd.cpu().numpy()
-    mask = np.ones(q.shape, dtype=bool)
-    mask[prob.interior()] = False
-    assert np.array_equal(after[mask], q[mask])
+    assert np.array_equal(after, ref)
 
 
 # ---------------------------------------------------------------------------------------------
@@ -198,9 +207,39 @@ def test_rhs_and_rk3_parity_mixed_boundary_kinds_on_the_fused_path(ndim, lo, hi,
     check_rk(prob_s, q_s, march_segment=8)
 
 
+# ---------------------------------------------------------------------------------------------
+# the two staging paths of the 3D kernel (TMA boxes / per-thread cp.async): every 3D instantiation, forced
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("nf", [1, 2, 3])
+@pytest.mark.parametrize("periodic", [True, False])
+@pytest.mark.parametrize("order", [5, 3, 1])
+def test_rhs_parity_tma_staging_and_bitwise_agreement_with_cp_async(nf, periodic, order):
+    """At an even padded extent both staging paths apply: each is held to the oracle, and they give the same bits
+    (same arithmetic on the same staged values).  Ragged tiles in x and y, several z segments."""
+    import dataclasses
+    prob, q = wl.random_state(3, (70, 29, 41), nf, seed=300 + nf, periodic=periodic)
+    prob = dataclasses.replace(prob, weno_order=order)
+    check_rhs(prob, q, march_segment=8, staging=B.MFC_STAGING_TMA)
+    with Gpu(prob, march_segment=8, staging=B.MFC_STAGING_TMA) as g1, Gpu(prob, march_segment=8, staging=B.MFC_STAGING_CPASYNC) as g2:
+        it = prob.interior()
+        assert np.array_equal(g1.rhs(q)[it], g2.rhs(q)[it])
+        orc = oracle.Oracle(prob)
+        dts = [0.5 * orc.cfl_dt(q.copy(), prob.cfl)] * 3
+        assert np.array_equal(g1.rk3(q, dts)[it], g2.rk3(q, dts)[it])
+
+
+def test_tma_staging_refuses_an_odd_padded_extent_and_auto_falls_back():
+    prob, q = wl.random_state(3, (33, 17, 9), 2, seed=5, periodic=True, rough=False)
+    with Gpu(prob, staging=B.MFC_STAGING_TMA) as g:
+        with pytest.raises(B.MfcError):
+            g.rhs(q)
+    check_rhs(prob, q, staging=B.MFC_STAGING_AUTO)
+
+
 @pytest.mark.parametrize("seg", [1, 5, 32, 1000])
-def test_rhs_is_independent_of_the_marching_segment(seg):
-    prob, q = wl.random_state(3, (40, 33, 37), 2, seed=77, periodic=False)
+@pytest.mark.parametrize("n0", [40, 41])
+def test_rhs_is_independent_of_the_marching_segment(seg, n0):
+    prob, q = wl.random_state(3, (n0, 33, 37), 2, seed=77, periodic=False)
     with Gpu(prob, march_segment=7) as g:
         ref = g.rhs(q)
     with Gpu(prob, march_segment=seg) as g:
@@ -514,8 +553,8 @@ def test_profile_hooks_count_launches_and_time():
         B.mfc_profile_enable(g.ctx, True)
         B.mfc_rk3_step(g.ctx, qd.data_ptr(), 1e-9, g.stream)
         B.mfc_cfl_dt(g.ctx, qd.data_ptr(), g.stream)
-        assert B.mfc_launch_count(g.ctx) - n0 == 3 + 1        # one fused launch per stage + the CFL reduction
-        for kid, want in [(B.MFC_K_RHS, 3), (B.MFC_K_CFL, 1)]:
+        assert B.mfc_launch_count(g.ctx) - n0 == 3 * 2 + 1    # per stage: ghost fill + one fused launch; the CFL reduction
+        for kid, want in [(B.MFC_K_RHS, 3), (B.MFC_K_GHOST, 3), (B.MFC_K_CFL, 1)]:
             n, ms = B.mfc_profile_get(g.ctx, kid, reset=True)
             assert n == want and ms > 0.0
         n, ms = B.mfc_profile_get(g.ctx, B.MFC_K_RHS)
