@@ -119,38 +119,41 @@ __device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, cons
     double *const FyH = B.HyL;                                      // [NEQ+1][FTX] over HyL, HyR[0]
 
     early();
-    // ---- rim states, one job per thread of the first four warps, one SIDE per warp (only that side of the
-    // reconstruction is evaluated): warp 0 left state of y face -1/2 (from row -1), warp 1 right state of the y face
-    // past the tile, warp 2 left state of x face -1/2 (from cell -1), warp 3 right states of the x face past the tile
-    // (lanes 0..15) and of x face -1/2 (lanes 16..31, from cell 0: recomputed here so that the rim face can be
-    // solved before lane 0 publishes it) ----
-    for (int job = tid; job < 128; job += NT) {
-        const bool inx = job >= 64;
-        if (!inx && D < 2) continue;
-        const bool left = inx ? job < 96 : job < 32;                // which side of the cell the state is taken from
-        const int r = inx ? (job & 15) : (job & 31);
-        const bool x0 = job >= 112;
-        if ((!inx || r < TY) && !(inx && left && (job & 31) >= 16)) {
-            const int st = inx ? 1 : FPX;                           // stride along the normal direction
-            const int cc = x0 ? 0 : (left ? -1 : (inx ? FTX : TY)); // centre cell along the normal direction
-            const double *pb = inx ? P + (r + HY) * FPX + NG + cc : P + (HY + cc) * FPX + NG + r;
-            double *dst = inx ? (x0 ? B.ExR : (left ? B.HxL : B.HxR)) + r : (left ? B.HyL : B.HyR) + r;
-            const int ds = inx ? TY : FTX;
-            double v, unused;
-            if (left) {
+    // ---- rim states.  A unit = ONE variable of one rim cell, one SIDE: (kind, variable e, index r along the rim) with
+    //   kind 0: left state of y face -1/2 (from row -1)          kind 1: right state of the y face past the tile (row TY)
+    //   kind 2: left state of x face -1/2 (from cell -1)         kind 3: right state of the x face past the tile (cell FTX)
+    //   kind 4: right state of x face -1/2 (from cell 0: recomputed here so that the rim face can be solved before lane 0
+    //           publishes it)
+    // dealt round-robin to ALL threads (two rounds in 3D with two fluids, the second one leaving out the two warps that
+    // solve the rim faces below), so that no warp reaches the barrier much later than the others.  A right state is the
+    // left state of the mirrored stencil: one code path, the side only flips the sign of the stride. ----
+    {
+        constexpr int UY = D >= 2 ? 2 * FTX * NEQ : 0, UX = 3 * TY * NEQ, U = UY + UX;
 #pragma unroll
-                for (int e = 0; e < NEQ; ++e) {
-                    const double *s5 = pb + e * PPL;
-                    reconstruct<ORDER>(s5[0], s5[-st] - s5[-2 * st], s5[0] - s5[-st], s5[st] - s5[0], s5[2 * st] - s5[st], eos.weno_eps4, v, unused);
-                    dst[e * ds] = v;
+        for (int u0 = 0; u0 < U; u0 += NT) {
+            const int u = u0 + tid;
+            if (u < U) {
+                int e, r, st;
+                const double *pb;
+                double *dst;
+                if (D >= 2 && u < UY) {
+                    const int kind = u / (FTX * NEQ), rem = u - kind * (FTX * NEQ);
+                    e = rem / FTX;
+                    r = rem - e * FTX;
+                    pb = P + e * PPL + (kind == 0 ? HY - 1 : HY + TY) * FPX + NG + r;
+                    st = kind == 0 ? FPX : -FPX;
+                    dst = (kind == 0 ? B.HyL : B.HyR) + e * FTX + r;
+                } else {
+                    const int v = u - UY, kind = v / (TY * NEQ), rem = v - kind * (TY * NEQ);
+                    e = rem / TY;
+                    r = rem - e * TY;
+                    pb = P + e * PPL + (r + HY) * FPX + NG + (kind == 0 ? -1 : (kind == 1 ? FTX : 0));
+                    st = kind == 0 ? 1 : -1;
+                    dst = (kind == 0 ? B.HxL : (kind == 1 ? B.HxR : B.ExR)) + e * TY + r;
                 }
-            } else {
-#pragma unroll
-                for (int e = 0; e < NEQ; ++e) {
-                    const double *s5 = pb + e * PPL;
-                    reconstruct<ORDER>(s5[0], s5[-st] - s5[-2 * st], s5[0] - s5[-st], s5[st] - s5[0], s5[2 * st] - s5[st], eos.weno_eps4, unused, v);
-                    dst[e * ds] = v;
-                }
+                double v, unused;
+                reconstruct<ORDER>(pb[0], pb[-st] - pb[-2 * st], pb[0] - pb[-st], pb[st] - pb[0], pb[2 * st] - pb[st], eos.weno_eps4, v, unused);
+                *dst = v;
             }
         }
     }
