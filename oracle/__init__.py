@@ -34,7 +34,23 @@ class _Problem(C.Structure):
         ("weno_eps", C.c_double),
         ("weno_order", C.c_int),
         ("kapila", C.c_int),
+        ("xe", C.POINTER(C.c_double) * 3),
     ]
+
+
+def padded_edges(edges, bc_lo: int, bc_hi: int) -> np.ndarray:
+    """Cell edges of the padded line from the n + 1 edges of the interior cells (non-uniform spacing).
+
+    A ghost cell has the width of the cell its value is copied from (reading B20b; the paper is silent):
+    periodic -> the widths wrap around; extrapolation -> the boundary cell's width repeated."""
+    e = np.asarray(edges, dtype=np.float64)
+    w = np.diff(e)
+    assert e.ndim == 1 and e.size >= NG + 1 and np.all(w > 0.0), "edges must increase"
+    lo = w[-NG:] if bc_lo == 0 else np.full(NG, w[0])
+    hi = w[:NG] if bc_hi == 0 else np.full(NG, w[-1])
+    left = e[0] - np.cumsum(lo[::-1])[::-1]
+    right = e[-1] + np.cumsum(hi)
+    return np.ascontiguousarray(np.concatenate([left, e, right]))
 
 
 STRICT_FLAGS = ["-O2", "-ffp-contract=off"]
@@ -97,6 +113,7 @@ def lib(path: Path | None = None):
         L.orc_rk3_step.argtypes = [pp, dp, C.c_double]; L.orc_rk3_step.restype = None
         L.orc_cfl_dt.argtypes = [pp, dp, C.c_double]; L.orc_cfl_dt.restype = C.c_double
         L.orc_weno3.argtypes = [C.c_double] * 4 + [dp, dp]; L.orc_weno3.restype = None
+        L.orc_weno5_nonuniform.argtypes = [dp, dp, C.c_double, dp, dp]; L.orc_weno5_nonuniform.restype = None
         L.orc_kapila_K.argtypes = [pp, C.c_double, C.c_double]; L.orc_kapila_K.restype = C.c_double
         L.orc_threads.argtypes = []; L.orc_threads.restype = C.c_int
         L.orc_set_threads.argtypes = [C.c_int]; L.orc_set_threads.restype = None
@@ -131,6 +148,16 @@ class Oracle:
         assert P.weno_order in (1, 3, 5)
         P.kapila = 1 if getattr(prob, "kapila", False) else 0
         assert not P.kapila or P.nf == 2, "the Kapila coefficient of Eq. 2 is the two-fluid one"
+        # non-uniform Cartesian spacing: prob.edges[d] = the n[d] + 1 edges of the interior cells, or None
+        self.xe = [None, None, None]
+        edges = getattr(prob, "edges", None)
+        for d in range(3):
+            P.xe[d] = None
+            if edges is not None and d < prob.ndim and edges[d] is not None:
+                assert P.weno_order in (1, 5), "non-uniform spacing: WENO5 (or first order) only"
+                assert len(edges[d]) == P.n[d] + 1
+                self.xe[d] = padded_edges(edges[d], P.bc_lo[d], P.bc_hi[d])
+                P.xe[d] = self.xe[d].ctypes.data_as(C.POINTER(C.c_double))
         self.P = P
         self.neq = self.L.orc_neq(C.byref(P))
         self.elems = self.L.orc_elems(C.byref(P))
@@ -196,6 +223,17 @@ def weno5(a, b, c, d, e, eps=1e-16):
     vL = C.c_double()
     vR = C.c_double()
     lib().orc_weno5(float(a), float(b), float(c), float(d), float(e), float(eps), C.byref(vL), C.byref(vR))
+    return vL.value, vR.value
+
+
+def weno5_nonuniform(xe, v, eps=1e-16):
+    """xe: the six edges of cells i-2..i+2, v: their five values -> (vL at x_{i+1/2}, vR at x_{i-1/2})."""
+    xe = np.ascontiguousarray(xe, dtype=np.float64)
+    v = np.ascontiguousarray(v, dtype=np.float64)
+    assert xe.size == 6 and v.size == 5
+    vL = C.c_double()
+    vR = C.c_double()
+    lib().orc_weno5_nonuniform(_dp(xe), _dp(v), float(eps), C.byref(vL), C.byref(vR))
     return vL.value, vR.value
 
 

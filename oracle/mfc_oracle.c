@@ -3,7 +3,7 @@
  *
  * Plain, slow, fp64 CPU statement of what the hot path computes: the right-hand side of the
  * 5-equation diffuse-interface model (Allaire, K = 0; optionally the Kapila source K div(u) of Eq. 2, two
- * fluids) with stiffened-gas EOS on a uniform grid,
+ * fluids) with stiffened-gas EOS on a uniform or non-uniform Cartesian grid (section A5c below),
  * driven by 3-stage TVD Runge-Kutta, exactly in the paper's order:
  *   ghost fill -> cons->prim -> per-direction WENO5-JS -> HLLC (+ face velocity) -> flux difference
  *   + alpha*div(u) -> RK stage combine;  plus the CFL time step.
@@ -47,6 +47,8 @@ typedef struct {
     double weno_eps;
     int weno_order;        /* 5 (WENO5-JS), 3 (WENO3-JS) or 1 (piecewise constant) */
     int kapila;            /* 0: Allaire model (K = 0); 1: Kapila source K div(u) on the alpha row, two fluids (Eq. 2) */
+    const double *xe[3];   /* non-uniform Cartesian spacing: xe[d] = the n[d] + 2 ng + 1 cell EDGES of the padded
+                              line of direction d (ghost cells included), increasing; NULL = uniform spacing dx[d] */
 } orc_problem;
 
 static int neq_of(const orc_problem *P) { return 2 * P->nf + P->ndim; }
@@ -210,6 +212,111 @@ void orc_reconstruct(const orc_problem *P, double a, double b, double c, double 
 }
 
 /* ------------------------------------------------------------------------------------------------
+ * A5c. WENO5-JS on a NON-UNIFORM grid ("structured mesh with non-uniform spacing"; Listing 1,
+ * PAPER.md:186-220, whose per-index tables poly_coef / beta_coef / d_cb are what the formulas below evaluate to;
+ * refs. [17] Jiang-Shu, [38] Shu for the general-stencil definitions; reading B20).  Written from the
+ * DEFINITIONS, cell by cell, with no tables:
+ *   - candidate r (r = 0, 1, 2: cells i-2..i, i-1..i+1, i..i+2) is the quadratic p_r whose cell averages over its three
+ *     cells are the data: p_r = V_r' with V_r the cubic Lagrange interpolant of the primitive function
+ *     V(x_{j+1/2}) = sum_{l <= j} v_l dx_l at the four edges of the stencil;
+ *   - beta_r = sum_{l=1,2} dx_i^(2l-1) int_{cell i} (d^l p_r / dx^l)^2 dx  (Jiang-Shu), which for the quadratic
+ *     p_r = a0 + a1 (x - x_i) + a2 (x - x_i)^2 is  a1^2 dx_i^2 + 13/3 a2^2 dx_i^4;
+ *   - the ideal weights at a face are the d_r with sum_r d_r p_r(face) = p5(face), p5 the quartic with the five cell
+ *     averages (V5' of the quintic interpolant at six edges): matching the coefficient of the outermost cells gives d_0 and
+ *     d_2, and d_1 = 1 - d_0 - d_2;
+ *   - alpha_r = d_r / (beta_r + eps)^2, omega_r = alpha_r / sum alpha, v = sum omega_r p_r(face)   (Eq. 12, Listing 1).
+ * On a uniform grid this is orc_weno5 (pinned to round-off).  xe: the six edges of cells i-2..i+2; v: the five cell values.
+ * ---------------------------------------------------------------------------------------------- */
+/* derivative at x of the Lagrange basis polynomial m over the nodes e[0..nn-1] */
+static double lagrange_d1(const double *e, int nn, int m, double x)
+{
+    double den = 1.0, sum = 0.0;
+    for (int l = 0; l < nn; ++l) if (l != m) den *= (e[m] - e[l]);
+    for (int l = 0; l < nn; ++l) {
+        if (l == m) continue;
+        double prod = 1.0;
+        for (int q = 0; q < nn; ++q) if (q != m && q != l) prod *= (x - e[q]);
+        sum += prod;
+    }
+    return sum / den;
+}
+/* second derivative at x of the CUBIC Lagrange basis polynomial m (four nodes) */
+static double lagrange4_d2(const double *e, int m, double x)
+{
+    double den = 1.0, sum = 0.0;
+    for (int l = 0; l < 4; ++l) if (l != m) { den *= (e[m] - e[l]); sum += (x - e[l]); }
+    return 2.0 * sum / den;
+}
+/* third derivative (a constant) of the cubic Lagrange basis polynomial m */
+static double lagrange4_d3(const double *e, int m)
+{
+    double den = 1.0;
+    for (int l = 0; l < 4; ++l) if (l != m) den *= (e[m] - e[l]);
+    return 6.0 / den;
+}
+/* value at x of the reconstruction polynomial (derivative of the interpolated primitive function) over the nc cells with
+ * edges e[0..nc], written as coefficients of the cell values: p(x) = sum_j coef[j] v_j,  coef[j] = dx_j sum_{m > j} l_m'(x) */
+static void recon_coef(const double *e, int nc, double x, double *coef)
+{
+    for (int j = 0; j < nc; ++j) {
+        double s = 0.0;
+        for (int m = j + 1; m <= nc; ++m) s += lagrange_d1(e, nc + 1, m, x);
+        coef[j] = (e[j + 1] - e[j]) * s;
+    }
+}
+
+void orc_weno5_nonuniform(const double *xe, const double *v, double eps, double *vL, double *vR)
+{
+    const double xm = xe[2], xp = xe[3];               /* faces i-1/2 and i+1/2 of the centre cell */
+    const double dxi = xp - xm, xc = 0.5 * (xm + xp);
+    double pL[3], pR[3], beta[3], c5L[5], c5R[5], dL[3], dR[3], cL[3][3], cR[3][3];
+    recon_coef(xe, 5, xp, c5L);
+    recon_coef(xe, 5, xm, c5R);
+    for (int r = 0; r < 3; ++r) {
+        const double *e = xe + r;                      /* four edges of cells i-2+r .. i+r */
+        const double *w = v + r;
+        recon_coef(e, 3, xp, cL[r]);
+        recon_coef(e, 3, xm, cR[r]);
+        pL[r] = cL[r][0] * w[0] + cL[r][1] * w[1] + cL[r][2] * w[2];
+        pR[r] = cR[r][0] * w[0] + cR[r][1] * w[1] + cR[r][2] * w[2];
+        /* primitive function at the four edges, V_0 = 0 */
+        double V[4] = { 0.0, 0.0, 0.0, 0.0 };
+        for (int m = 1; m < 4; ++m) V[m] = V[m - 1] + w[m - 1] * (e[m] - e[m - 1]);
+        double a1 = 0.0, a2 = 0.0;                     /* p_r = a0 + a1 (x - xc) + a2 (x - xc)^2 */
+        for (int m = 0; m < 4; ++m) {
+            a1 += V[m] * lagrange4_d2(e, m, xc);
+            a2 += 0.5 * V[m] * lagrange4_d3(e, m);
+        }
+        beta[r] = a1 * a1 * dxi * dxi + 13.0 / 3.0 * a2 * a2 * dxi * dxi * dxi * dxi;
+    }
+    /* ideal weights: stencil 0 alone reaches cell i-2, stencil 2 alone reaches cell i+2 */
+    dL[0] = c5L[0] / cL[0][0]; dL[2] = c5L[4] / cL[2][2]; dL[1] = 1.0 - dL[0] - dL[2];
+    dR[0] = c5R[0] / cR[0][0]; dR[2] = c5R[4] / cR[2][2]; dR[1] = 1.0 - dR[0] - dR[2];
+    {
+        double a[3], s = 0.0;
+        for (int r = 0; r < 3; ++r) { a[r] = dL[r] / ((beta[r] + eps) * (beta[r] + eps)); s += a[r]; }
+        *vL = (a[0] / s) * pL[0] + (a[1] / s) * pL[1] + (a[2] / s) * pL[2];
+    }
+    {
+        double a[3], s = 0.0;
+        for (int r = 0; r < 3; ++r) { a[r] = dR[r] / ((beta[r] + eps) * (beta[r] + eps)); s += a[r]; }
+        *vR = (a[0] / s) * pR[0] + (a[1] / s) * pR[1] + (a[2] / s) * pR[2];
+    }
+}
+
+/* the reconstruction of cell j (padded index) of a line of direction dir: uniform or non-uniform */
+static void reconstruct_at(const orc_problem *P, int dir, int jpad, const double *st, double *vL, double *vR)
+{
+    if (P->xe[dir] && P->weno_order == 5) orc_weno5_nonuniform(P->xe[dir] + jpad - 2, st, P->weno_eps, vL, vR);
+    else orc_reconstruct(P, st[0], st[1], st[2], st[3], st[4], vL, vR);
+}
+/* width of cell j (padded index) in direction dir */
+static double cell_width(const orc_problem *P, int dir, int jpad)
+{
+    return P->xe[dir] ? P->xe[dir][jpad + 1] - P->xe[dir][jpad] : P->dx[dir];
+}
+
+/* ------------------------------------------------------------------------------------------------
  * A6. HLLC, PAPER.md:152-164 (Eq. 13-14), with the face velocity of PAPER.md:126-136 (Eq. 10 and the
  * garbled equation after section 3.2: the Riemann solver returns F and u; reading B5).
  *   s_L = min(u_L - c_L, u_R - c_R), s_R = max(u_L + c_L, u_R + c_R)                  (reading B11)
@@ -326,8 +433,7 @@ void orc_rhs(const orc_problem *P, double *q, double *L)
                         idx[dir] = ORC_NG + j + s;
                         st[s + 2] = w[(size_t)e * C + at(P, idx[0], idx[1], idx[2])];
                     }
-                    orc_reconstruct(P, st[0], st[1], st[2], st[3], st[4],
-                                    &vL[(size_t)(j + 1) * neq + e], &vR[(size_t)(j + 1) * neq + e]);
+                    reconstruct_at(P, dir, ORC_NG + j, st, &vL[(size_t)(j + 1) * neq + e], &vR[(size_t)(j + 1) * neq + e]);
                 }
             }
             /* HLLC: faces f = j+1/2, j = -1..n-1; left state from cell j, right state from cell j+1
@@ -340,12 +446,13 @@ void orc_rhs(const orc_problem *P, double *q, double *L)
                 size_t cell;
                 idx[dir] = ORC_NG + j;
                 cell = at(P, idx[0], idx[1], idx[2]);
+                const double dxj = cell_width(P, dir, ORC_NG + j);            /* Eq. 8-9: the cell's own width */
                 for (int e = 0; e < neq; ++e)
-                    L[(size_t)e * C + cell] += (Ff[(size_t)j * neq + e] - Ff[(size_t)(j + 1) * neq + e]) / P->dx[dir];
+                    L[(size_t)e * C + cell] += (Ff[(size_t)j * neq + e] - Ff[(size_t)(j + 1) * neq + e]) / dxj;
                 for (int i = 0; i < nf - 1; ++i) {
                     double h = q[(size_t)(iA + i) * C + cell];
                     if (P->kapila && nf == 2) h += orc_kapila_K(P, w[(size_t)iA * C + cell], w[(size_t)(nf + D) * C + cell]);
-                    L[(size_t)(iA + i) * C + cell] += h * (uf[j + 1] - uf[j]) / P->dx[dir];
+                    L[(size_t)(iA + i) * C + cell] += h * (uf[j + 1] - uf[j]) / dxj;
                 }
             }
             free(vL); free(vR); free(Ff); free(uf);
@@ -363,7 +470,7 @@ void orc_line(const orc_problem *P, int dir, int n, const double *w, double *vL,
     for (int j = -1; j <= n; ++j)
         for (int e = 0; e < neq; ++e) {
             const double *s = w + (size_t)e * np + ORC_NG + j;
-            orc_reconstruct(P, s[-2], s[-1], s[0], s[1], s[2], &vL[(size_t)e * (n + 2) + j + 1], &vR[(size_t)e * (n + 2) + j + 1]);
+            reconstruct_at(P, dir, ORC_NG + j, s - 2, &vL[(size_t)e * (n + 2) + j + 1], &vR[(size_t)e * (n + 2) + j + 1]);
         }
     for (int j = -1; j <= n - 1; ++j) {
         double wl[ORC_MAXEQ], wr[ORC_MAXEQ], f[ORC_MAXEQ];
@@ -398,7 +505,7 @@ void orc_rk3_step(const orc_problem *P, double *q, double dt)
 
 /* ------------------------------------------------------------------------------------------------
  * A9. CFL time step ("CFL-restricted time step"; reading B17):
- *   dt = cfl * min over interior cells and directions of dx_d / (|u_d| + c).
+ *   dt = cfl * min over interior cells and directions of dx_d / (|u_d| + c), dx_d the cell's own width.
  * ---------------------------------------------------------------------------------------------- */
 double orc_cfl_dt(const orc_problem *P, const double *q, double cfl)
 {
@@ -416,7 +523,8 @@ double orc_cfl_dt(const orc_problem *P, const double *q, double cfl)
                 mixture(P, w + nf + D + 1, &Gam, &Pi);
                 c = sqrt(((Gam + 1.0) * w[nf + D] + Pi) / (Gam * rho));
                 for (int d = 0; d < D; ++d) {
-                    double t = P->dx[d] / (fabs(w[nf + d]) + c);
+                    const int jp = (d == 0 ? i : d == 1 ? j : k) + ORC_NG;
+                    double t = cell_width(P, d, jp) / (fabs(w[nf + d]) + c);
                     if (t < best) best = t;
                 }
             }

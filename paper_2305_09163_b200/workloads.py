@@ -54,6 +54,8 @@ class Problem:
     notes: str = ""
     weno_order: int = 5  # 5: WENO5-JS (the paper's default), 3: WENO3-JS, 1: piecewise constant
     kapila: bool = False  # K div(u) source of PAPER.md Eq. 2 on the alpha row (two fluids); False = Allaire
+    # non-uniform Cartesian spacing: per dimension the n + 1 edges of the interior cells, or None (uniform)
+    edges: Tuple | None = None
 
     @property
     def nf(self) -> int:
@@ -84,13 +86,48 @@ class Problem:
         return (slice(None), sl[2], sl[1], sl[0])
 
     def centers(self, d: int) -> np.ndarray:
+        if self.edges is not None and self.edges[d] is not None:
+            e = np.asarray(self.edges[d], dtype=np.float64)
+            return 0.5 * (e[:-1] + e[1:])
         h = self.dx[d]
         return self.lo[d] + (np.arange(self.n[d], dtype=np.float64) + 0.5) * h
+
+    def widths(self, d: int) -> np.ndarray:
+        """Widths of the interior cells of dimension d."""
+        if self.edges is not None and self.edges[d] is not None:
+            return np.diff(np.asarray(self.edges[d], dtype=np.float64))
+        return np.full(self.n[d], self.dx[d])
 
 
 def _grid(ndim: int, n: Sequence[int]) -> Tuple[Tuple[int, int, int], Tuple[float, ...], Tuple[float, ...]]:
     nn = tuple(int(n[d]) if d < ndim else 1 for d in range(3))
     return nn, (0.0, 0.0, 0.0), (1.0, 1.0, 1.0)
+
+
+def stretched_edges(n: int, lo: float = 0.0, hi: float = 1.0, a: float = 4.0, xa: float = -0.12, xb: float = 0.12) -> np.ndarray:
+    """The n + 1 cell edges of a grid refined near the middle of [lo, hi] by the hyperbolic-tangent stretching of
+    PAPER.md:396-399 (Eq. 15), applied to the uniform edges in the centred coordinate x = (xi - mid) (the paper's droplet
+    sits at the origin, x_a = -1.2 D, x_b = 1.2 D, a_x = 4):
+        x_s = x + (x / a) [log cosh(a (x - x_a) / L) + log cosh(a (x - x_b) / L) - 2 log cosh(a (x_b - x_a) / (2 L))]
+    L = hi - lo.  Cells at the ends are about 2.6 x wider than in the middle for the defaults.  Input definition only."""
+    L = hi - lo
+    mid = 0.5 * (lo + hi)
+    x = np.linspace(lo, hi, n + 1) - mid
+    lc = lambda t: np.log(np.cosh(t))
+    xs = x + (x / a) * (lc(a * (x - xa) / L) + lc(a * (x - xb) / L) - 2.0 * lc(a * (xb - xa) / (2.0 * L)))
+    assert np.all(np.diff(xs) > 0.0)
+    return xs + mid
+
+
+def with_stretched_grid(prob: Problem, dims=None, **kw) -> Problem:
+    """The same problem on the Eq. 15 grid in the given dimensions (default: all active ones).  Initial data are defined
+    per cell index, so the state array is reused as it is: same per-cell values on the stretched cells."""
+    import dataclasses
+    dims = range(prob.ndim) if dims is None else dims
+    edges = [None, None, None]
+    for d in dims:
+        edges[d] = stretched_edges(prob.n[d], prob.lo[d], prob.hi[d], **kw)
+    return dataclasses.replace(prob, name=prob.name + "_stretched", edges=tuple(edges))
 
 
 def assemble(prob: Problem, alpha: Sequence[np.ndarray], rho_i: Sequence, vel: Sequence, p) -> np.ndarray:
