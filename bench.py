@@ -176,6 +176,9 @@ def run_ours(args):
     if args.kapila:
         import dataclasses
         prob = dataclasses.replace(prob, name=prob.name + "+kapila", kapila=True)
+    if args.stretched:
+        from paper_2305_09163_b200 import workloads as wl
+        prob = wl.with_stretched_grid(prob)
     ctx = B.init_from_problem(prob, device=local, march_segment=args.segment)
     neq, ng, padded, elems = B.mfc_layout(ctx)
     stream = torch.cuda.current_stream().cuda_stream
@@ -348,6 +351,7 @@ def main():
     ap.add_argument("--ref-n", type=int, default=96, help="cells per dimension of the --impl reference sample")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--kapila", action="store_true", help="switch the K div(u) source of PAPER.md Eq. 2 on (not the headline config)")
+    ap.add_argument("--stretched", action="store_true", help="same per-cell data on the Eq. 15 stretched grid (non-uniform spacing; not the headline config)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -1,6 +1,6 @@
 /*
  * mfc.h -- C ABI of libmfc_b200: the right-hand side of the 5-equation diffuse-interface model
- * (Allaire form, K = 0) with stiffened-gas EOS on a uniform structured grid, as hand-written CUDA for
+ * (Allaire form, K = 0) with stiffened-gas EOS on a uniform or non-uniform Cartesian grid, as hand-written CUDA for
  * sm_100a (NVIDIA B200), driven by 3-stage TVD Runge-Kutta.
  *
  * Method: arxiv 2305.09163 (Radhakrishnan et al.), cited below as PAPER.md:LINE (section / equation).
@@ -46,16 +46,23 @@ extern "C" {
 typedef enum {
     MFC_OK = 0,
     MFC_EINVAL = -1,       /* null pointer, bad shape, n_d < 3 in an active dimension, gamma <= 1, bad BC kind or order */
-    MFC_EUNSUPPORTED = -2, /* (ndim, n_fluids) outside the compiled template set; kapila with n_fluids != 2 */
+    MFC_EUNSUPPORTED = -2, /* (ndim, n_fluids) outside the compiled template set; kapila with n_fluids != 2; non-uniform
+                              spacing with weno_order != 5 or with a non-positive ideal weight */
     MFC_ECUDA = -3,        /* CUDA runtime error (sticky); no device */
     MFC_ENOMEM = -4        /* device or host allocation failed */
 } mfc_status;
 
-/* uniform grid, PAPER.md:105-124 (Eq. 6-9): dx_d = (hi_d - lo_d) / n_d */
+/* Cartesian grid, PAPER.md:105-124 (Eq. 6-9).  Uniform by default: dx_d = (hi_d - lo_d) / n_d.
+ * Non-uniform spacing ("structured mesh with non-uniform spacing"; Listing 1's per-index coefficient tables;
+ * Eq. 15 stretching): edges_host[d] != NULL gives the n[d] + 1 strictly increasing cell edges of dimension d (host
+ * pointer, copied by mfc_init; lo[d], hi[d] are then ignored); dimensions may be mixed.  A ghost cell has the width of the
+ * cell its value is copied from (periodic: widths wrap; extrapolation: the boundary cell's width).  WENO5 only
+ * (weno_order 5); the ideal weights of every cell must be positive (true for smooth stretching), else MFC_EUNSUPPORTED. */
 typedef struct {
     int ndim;        /* 1, 2 or 3 */
     int n[3];        /* interior cells; entries >= ndim are ignored (treated as 1) */
     double lo[3], hi[3];
+    const double *edges_host[3]; /* NULL: uniform in that dimension */
 } mfc_grid;
 
 /* stiffened gas, PAPER.md:54-58 (Eq. 1) */
@@ -130,7 +137,8 @@ int mfc_cons_to_prim(mfc_ctx *ctx, const double *q_dev, double *w_dev, void *str
 
 /* a2 + a3 on one line of primitives with normal direction dir (0,1,2 < ndim), using the same device
  * functions as the sweeps.  w_dev: [neq][n + 6]; vL_dev, vR_dev: [neq][n + 2] (cells -1..n: state at face
- * i+1/2 resp. i-1/2 seen from cell i); F_dev: [neq][n + 1]; uface_dev: [n + 1] (faces -1/2 .. n-1/2). */
+ * i+1/2 resp. i-1/2 seen from cell i); F_dev: [neq][n + 1]; uface_dev: [n + 1] (faces -1/2 .. n-1/2).
+ * On a non-uniform grid the line is one of the grid's own lines of that direction: n must equal n[dir]. */
 int mfc_line_fluxes(mfc_ctx *ctx, int dir, int n, const double *w_dev, double *vL_dev, double *vR_dev,
                     double *F_dev, double *uface_dev, void *stream);
 

@@ -39,7 +39,8 @@ class MfcError(RuntimeError):
 
 
 class mfc_grid(C.Structure):
-    _fields_ = [("ndim", C.c_int), ("n", C.c_int * 3), ("lo", C.c_double * 3), ("hi", C.c_double * 3)]
+    _fields_ = [("ndim", C.c_int), ("n", C.c_int * 3), ("lo", C.c_double * 3), ("hi", C.c_double * 3),
+                ("edges_host", C.POINTER(C.c_double) * 3)]
 
 
 class mfc_fluid(C.Structure):
@@ -107,8 +108,9 @@ def mfc_version() -> str:
 
 
 def mfc_init(grid_n, lo, hi, fluids, bc_lo, bc_hi, *, weno_eps=1e-16, cfl=0.3, device=-1, march_segment=0, weno_order=5,
-             kapila=False, staging=MFC_STAGING_AUTO):
-    """grid_n / lo / hi: one entry per active dimension; fluids: [(gamma, pi_inf), ...]; returns the context handle."""
+             kapila=False, staging=MFC_STAGING_AUTO, edges=None):
+    """grid_n / lo / hi: one entry per active dimension; fluids: [(gamma, pi_inf), ...]; edges: per dimension the
+    n + 1 cell edges (any sequence of floats) or None for uniform spacing; returns the context handle."""
     ndim = len(grid_n)
     g = mfc_grid()
     g.ndim = ndim
@@ -119,6 +121,15 @@ def mfc_init(grid_n, lo, hi, fluids, bc_lo, bc_hi, *, weno_eps=1e-16, cfl=0.3, d
         g.hi[d] = float(hi[d]) if d < ndim else 1.0
         b.lo[d] = int(bc_lo[d]) if d < ndim else MFC_BC_EXTRAP
         b.hi[d] = int(bc_hi[d]) if d < ndim else MFC_BC_EXTRAP
+    keep = []                                    # host edge arrays, alive until mfc_init has copied them
+    for d in range(3):
+        e = edges[d] if edges is not None and d < ndim and d < len(edges) else None
+        if e is None:
+            g.edges_host[d] = None
+        else:
+            arr = (C.c_double * (int(grid_n[d]) + 1))(*[float(v) for v in e])
+            keep.append(arr)
+            g.edges_host[d] = C.cast(arr, C.POINTER(C.c_double))
     fl = (mfc_fluid * max(1, len(fluids)))()
     for i, (gam, pinf) in enumerate(fluids):
         fl[i].gamma, fl[i].pi_inf = float(gam), float(pinf)
@@ -208,4 +219,4 @@ def init_from_problem(prob, **kw):
     D = prob.ndim
     return mfc_init(prob.n[:D], prob.lo[:D], prob.hi[:D], prob.fluids, prob.bc_lo[:D], prob.bc_hi[:D],
                     weno_eps=prob.weno_eps, cfl=prob.cfl, weno_order=getattr(prob, "weno_order", 5),
-                    kapila=getattr(prob, "kapila", False), **kw)
+                    kapila=getattr(prob, "kapila", False), edges=getattr(prob, "edges", None), **kw)

@@ -22,7 +22,7 @@ cudaError_t launch_prim(int ndim, int nf, const Geo &g, const Eos &e, const doub
     }
     return cudaErrorInvalidValue;
 }
-cudaError_t launch_rhs(int ndim, int nf, int order, const Geo &g, const Eos &e, const double *q, const SweepOut &o, int segment,
+cudaError_t launch_rhs(int ndim, int nf, int order, const GeoNu &g, const Eos &e, const double *q, const SweepOut &o, int segment,
                        int path, cudaStream_t s)
 {
     switch (ndim) {
@@ -32,7 +32,7 @@ cudaError_t launch_rhs(int ndim, int nf, int order, const Geo &g, const Eos &e, 
     }
     return cudaErrorInvalidValue;
 }
-cudaError_t launch_cfl(int ndim, int nf, const Geo &g, const Eos &e, const double *q, unsigned long long *min_bits,
+cudaError_t launch_cfl(int ndim, int nf, const GeoNu &g, const Eos &e, const double *q, unsigned long long *min_bits,
                        cudaStream_t s)
 {
     switch (ndim) {
@@ -43,12 +43,12 @@ cudaError_t launch_cfl(int ndim, int nf, const Geo &g, const Eos &e, const doubl
     return cudaErrorInvalidValue;
 }
 cudaError_t launch_line(int ndim, int nf, int order, int dir, const Eos &e, int n, const double *w, double *vL, double *vR,
-                        double *F, double *uf, cudaStream_t s)
+                        double *F, double *uf, const double *nu, int nus, cudaStream_t s)
 {
     switch (ndim) {
-        case 1: return launch_line_d1(nf, order, dir, e, n, w, vL, vR, F, uf, s);
-        case 2: return launch_line_d2(nf, order, dir, e, n, w, vL, vR, F, uf, s);
-        case 3: return launch_line_d3(nf, order, dir, e, n, w, vL, vR, F, uf, s);
+        case 1: return launch_line_d1(nf, order, dir, e, n, w, vL, vR, F, uf, nu, nus, s);
+        case 2: return launch_line_d2(nf, order, dir, e, n, w, vL, vR, F, uf, nu, nus, s);
+        case 3: return launch_line_d3(nf, order, dir, e, n, w, vL, vR, F, uf, nu, nus, s);
     }
     return cudaErrorInvalidValue;
 }
@@ -139,9 +139,10 @@ struct mfc_ctx {
     int ndim = 0, nf = 0, neq = 0, device = 0, segment = 0, order = 5, staging = 0;
     double cfl = 0.3;
     long long elems = 0;
-    mfc::Geo g{};
+    mfc::GeoNu g{};
     mfc::Eos e{};
     double *q1 = nullptr, *q2 = nullptr, *q_own = nullptr;
+    double *nu_dev[3] = {nullptr, nullptr, nullptr};   // non-uniform spacing: per-direction coefficient tables
     unsigned long long *min_dev = nullptr;
     unsigned long long *min_host = nullptr;  // pinned
     bool profile = false;
@@ -283,6 +284,107 @@ __global__ void __launch_bounds__(256) dfma_probe_kernel(double *out, int iters,
     out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
 }
 
+
+// ---------------------------------------------------------------------------------------------------------
+// Non-uniform spacing: the per-index coefficient tables of Listing 1 (poly_coef, beta_coef, d_cb), built
+// once per context on the host.  The reconstruction polynomial of a stencil is the derivative of the Newton interpolant
+// (divided differences) of the primitive function of the cell averages at the stencil's edges (refs. [17], [38]); every
+// table entry is that polynomial, or one of its derivatives, applied to a unit datum.
+// ---------------------------------------------------------------------------------------------------------
+// d^k/dx^k at x (k = 1, 2, 3) of the Newton interpolant of V(e_m) = sum_{l < m} u_l (e_{l+1} - e_l), nc cells, nc + 1 edges
+double newton_primitive_deriv(const double *e, int nc, const double *u, double x, int k)
+{
+    double dd[8];
+    dd[0] = 0.0;
+    for (int m = 1; m <= nc; ++m) dd[m] = dd[m - 1] + u[m - 1] * (e[m] - e[m - 1]);
+    for (int lev = 1; lev <= nc; ++lev)
+        for (int m = nc; m >= lev; --m) dd[m] = (dd[m] - dd[m - 1]) / (e[m] - e[m - lev]);
+    // omega_m = prod_{l < m} (x - e_l) and its first three derivatives, by the product rule
+    double w0 = 1.0, w1 = 0.0, w2 = 0.0, w3 = 0.0, res = 0.0;
+    for (int m = 0; m <= nc; ++m) {
+        res += dd[m] * (k == 1 ? w1 : (k == 2 ? w2 : w3));
+        const double f = x - e[m];
+        w3 = w3 * f + 3.0 * w2;
+        w2 = w2 * f + 2.0 * w1;
+        w1 = w1 * f + w0;
+        w0 = w0 * f;
+    }
+    return res;
+}
+
+// padded edges from the interior ones: a ghost cell has the width of the cell its value comes from (mfc.h)
+std::vector<double> padded_edges(const double *edges, int n, int bc_lo, int bc_hi)
+{
+    std::vector<double> xe(n + 2 * NG + 1);
+    for (int i = 0; i <= n; ++i) xe[NG + i] = edges[i];
+    for (int m = 1; m <= NG; ++m) {
+        const int sl = bc_lo == MFC_BC_PERIODIC ? n - m : 0;            // interior cell the ghost cell -m copies
+        const int sh = bc_hi == MFC_BC_PERIODIC ? m - 1 : n - 1;        // ... and the ghost cell n - 1 + m
+        xe[NG - m] = xe[NG - m + 1] - (edges[sl + 1] - edges[sl]);
+        xe[NG + n + m] = xe[NG + n + m - 1] + (edges[sh + 1] - edges[sh]);
+    }
+    return xe;
+}
+
+// table [NU_NC][stride] of one direction; false if an ideal weight is not positive
+bool nu_tables(const std::vector<double> &xe, int p, int stride, std::vector<double> &tab)
+{
+    tab.assign((size_t)NU_NC * stride, 0.0);
+    bool ok = true;
+    for (int j = 2; j <= p - 3; ++j) {
+        const double xm = xe[j], xp = xe[j + 1], h = xp - xm, xc = 0.5 * (xm + xp);
+        double *t = tab.data() + j;
+        auto put = [&](int k, double v) { t[(size_t)k * stride] = v; };
+        double dL[3], dR[3], pL[3][2], pR[3][2];
+        const double e5[5][5] = {{1, 0, 0, 0, 0}, {0, 1, 0, 0, 0}, {0, 0, 1, 0, 0}, {0, 0, 0, 1, 0}, {0, 0, 0, 0, 1}};
+        for (int r = 0; r < 3; ++r) {
+            const double *e = &xe[j - 2 + r];
+            const int lc = 2 - r;                                       // the centre cell within the stencil
+            const double uA[3] = {0, 1, 1}, uB[3] = {0, 0, 1};          // unit differences: (d1, d2) = (1, 0) and (0, 1)
+            pL[r][0] = newton_primitive_deriv(e, 3, uA, xp, 1) - uA[lc];
+            pL[r][1] = newton_primitive_deriv(e, 3, uB, xp, 1) - uB[lc];
+            pR[r][0] = newton_primitive_deriv(e, 3, uA, xm, 1) - uA[lc];
+            pR[r][1] = newton_primitive_deriv(e, 3, uB, xm, 1) - uB[lc];
+            // p_r = a0 + a1 (x - xc) + a2 (x - xc)^2:  a1 = p'(xc), a2 = p'' / 2;  beta = a1^2 h^2 + 13/3 a2^2 h^4 (Jiang-Shu)
+            const double l1 = newton_primitive_deriv(e, 3, uA, xc, 2), l2 = newton_primitive_deriv(e, 3, uB, xc, 2);
+            const double m1 = 0.5 * newton_primitive_deriv(e, 3, uA, xc, 3), m2 = 0.5 * newton_primitive_deriv(e, 3, uB, xc, 3);
+            const double h2 = h * h, h4 = h2 * h2;
+            put(3 * r + 0, h2 * l1 * l1 + 13.0 / 3.0 * h4 * m1 * m1);
+            put(3 * r + 1, 2.0 * h2 * l1 * l2 + 26.0 / 3.0 * h4 * m1 * m2);
+            put(3 * r + 2, h2 * l2 * l2 + 13.0 / 3.0 * h4 * m2 * m2);
+        }
+        // ideal weights: the combination of the three quadratics that equals the five-cell quartic at the face; the outermost
+        // cells belong to one stencil each
+        const double *e5e = &xe[j - 2];
+        const double u3first[3] = {1, 0, 0}, u3last[3] = {0, 0, 1};
+        for (int side = 0; side < 2; ++side) {
+            const double x = side == 0 ? xp : xm;
+            double *d = side == 0 ? dL : dR;
+            d[0] = newton_primitive_deriv(e5e, 5, e5[0], x, 1) / newton_primitive_deriv(&xe[j - 2], 3, u3first, x, 1);
+            d[2] = newton_primitive_deriv(e5e, 5, e5[4], x, 1) / newton_primitive_deriv(&xe[j], 3, u3last, x, 1);
+            d[1] = 1.0 - d[0] - d[2];
+            for (int r = 0; r < 3; ++r) ok = ok && d[r] > 0.0;
+        }
+        for (int r = 0; r < 3; ++r) {
+            put(9 + 2 * r, dL[r] * pL[r][0]);
+            put(10 + 2 * r, dL[r] * pL[r][1]);
+            put(15 + 2 * r, dR[r] * pR[r][0]);
+            put(16 + 2 * r, dR[r] * pR[r][1]);
+            put(21 + r, dL[r]);
+            put(24 + r, dR[r]);
+        }
+        put(27, 1.0 / h);
+    }
+    // entries without a full stencil and the padding past the last cell: copies of the nearest valid cell (read by threads
+    // that write nothing, never used)
+    for (int k = 0; k < NU_NC; ++k) {
+        double *row = tab.data() + (size_t)k * stride;
+        for (int j = 0; j < 2 && j < stride; ++j) row[j] = row[2];
+        for (int j = p - 2; j < stride; ++j) row[j] = row[p - 3];
+    }
+    return ok;
+}
+
 }  // namespace
 
 extern "C" {
@@ -313,12 +415,19 @@ int mfc_init(mfc_ctx **out, const mfc_grid *grid, int n_fluids, const mfc_fluid 
     const int order = (opts && opts->weno_order != 0) ? opts->weno_order : 5;
     if (order != 1 && order != 3 && order != 5) return MFC_EINVAL;
     if (opts && (opts->staging < 0 || opts->staging > 2)) return MFC_EINVAL;
+    bool nonuniform = false;
     for (int d = 0; d < grid->ndim; ++d) {
-        if (grid->n[d] < MFC_NG || !(grid->hi[d] > grid->lo[d])) return MFC_EINVAL;
+        if (grid->n[d] < MFC_NG) return MFC_EINVAL;
+        if (grid->edges_host[d]) {
+            nonuniform = true;
+            for (int i = 0; i < grid->n[d]; ++i)
+                if (!(grid->edges_host[d][i + 1] > grid->edges_host[d][i]) || !std::isfinite(grid->edges_host[d][i + 1] - grid->edges_host[d][i])) return MFC_EINVAL;
+        } else if (!(grid->hi[d] > grid->lo[d])) return MFC_EINVAL;
         if (bc->lo[d] != MFC_BC_PERIODIC && bc->lo[d] != MFC_BC_EXTRAP) return MFC_EINVAL;
         if (bc->hi[d] != MFC_BC_PERIODIC && bc->hi[d] != MFC_BC_EXTRAP) return MFC_EINVAL;
         if ((bc->lo[d] == MFC_BC_PERIODIC) != (bc->hi[d] == MFC_BC_PERIODIC)) return MFC_EINVAL;
     }
+    if (nonuniform && order != 5) return MFC_EUNSUPPORTED;
     for (int i = 0; i < n_fluids; ++i)
         if (!(eos[i].gamma > 1.0) || !std::isfinite(eos[i].gamma) || !std::isfinite(eos[i].pi_inf)) return MFC_EINVAL;
 
@@ -338,14 +447,14 @@ int mfc_init(mfc_ctx **out, const mfc_grid *grid, int n_fluids, const mfc_fluid 
     c->order = order;
     const double eps = (opts && opts->weno_eps > 0.0) ? opts->weno_eps : 1.0e-16;
 
-    Geo &g = c->g;
+    GeoNu &g = c->g;
     g.ndim = grid->ndim;
     for (int d = 0; d < 3; ++d) {
         const bool act = d < grid->ndim;
         g.n[d] = act ? grid->n[d] : 1;
         g.g[d] = act ? NG : 0;
         g.p[d] = g.n[d] + 2 * g.g[d];
-        g.inv_dx[d] = act ? (double)grid->n[d] / (grid->hi[d] - grid->lo[d]) : 1.0;
+        g.inv_dx[d] = act && !grid->edges_host[d] ? (double)grid->n[d] / (grid->hi[d] - grid->lo[d]) : 1.0;
         g.bc_lo[d] = act ? bc->lo[d] : MFC_BC_EXTRAP;
         g.bc_hi[d] = act ? bc->hi[d] : MFC_BC_EXTRAP;
     }
@@ -391,6 +500,30 @@ int mfc_init(mfc_ctx **out, const mfc_grid *grid, int n_fluids, const mfc_fluid 
         if (err == cudaSuccess) err = cudaMemcpy(e.ygm1, tmp + MAX_NF, MAX_NF * sizeof(double), cudaMemcpyDeviceToHost);
         cudaFree(tmp);
     }
+    // non-uniform spacing: coefficient tables of every active dimension (a uniform dimension of a mixed grid gets the
+    // tables of its uniform edges), rows padded so that ragged tiles read defined entries
+    for (int d = 0; d < 3; ++d) { g.nu[d] = nullptr; g.nus[d] = 0; }
+    if (err == cudaSuccess && nonuniform) {
+        for (int d = 0; d < grid->ndim && err == cudaSuccess; ++d) {
+            std::vector<double> uni;
+            const double *edges = grid->edges_host[d];
+            if (!edges) {
+                uni.resize(grid->n[d] + 1);
+                for (int i = 0; i <= grid->n[d]; ++i) uni[i] = grid->lo[d] + (grid->hi[d] - grid->lo[d]) * ((double)i / grid->n[d]);
+                edges = uni.data();
+            }
+            const std::vector<double> xe = padded_edges(edges, grid->n[d], bc->lo[d], bc->hi[d]);
+            std::vector<double> tab;
+            g.nus[d] = g.p[d] + 64;
+            if (!nu_tables(xe, g.p[d], g.nus[d], tab)) {
+                mfc_destroy(c);
+                return MFC_EUNSUPPORTED;
+            }
+            err = cudaMalloc((void **)&c->nu_dev[d], tab.size() * sizeof(double));
+            if (err == cudaSuccess) err = cudaMemcpy(c->nu_dev[d], tab.data(), tab.size() * sizeof(double), cudaMemcpyHostToDevice);
+            g.nu[d] = c->nu_dev[d];
+        }
+    }
     if (err != cudaSuccess) {
         const int st = cuda_to_status(err);
         cudaGetLastError();
@@ -411,6 +544,7 @@ void mfc_destroy(mfc_ctx *c)
         cudaFree(c->q1);
         cudaFree(c->q2);
         cudaFree(c->q_own);
+        for (int d = 0; d < 3; ++d) cudaFree(c->nu_dev[d]);
         cudaFree(c->min_dev);
         if (c->min_host) cudaFreeHost(c->min_host);
     }
@@ -500,7 +634,9 @@ int mfc_line_fluxes(mfc_ctx *c, int dir, int n, const double *w_dev, double *vL_
     if (!c || !w_dev || !vL_dev || !vR_dev || !F_dev || !uface_dev || n < 1 || dir < 0 || dir >= c->ndim) return MFC_EINVAL;
     DeviceGuard guard(c->device);
     c->launch_total += 2;
-    return cuda_to_status(launch_line(c->ndim, c->nf, c->order, dir, c->e, n, w_dev, vL_dev, vR_dev, F_dev, uface_dev, (cudaStream_t)stream));
+    if (c->g.nu[0] && n != c->g.n[dir]) return MFC_EINVAL;     // the tables are those of the grid's own lines
+    return cuda_to_status(launch_line(c->ndim, c->nf, c->order, dir, c->e, n, w_dev, vL_dev, vR_dev, F_dev, uface_dev, c->g.nu[dir], c->g.nus[dir],
+                                      (cudaStream_t)stream));
 }
 
 int mfc_profile_enable(mfc_ctx *c, int on)

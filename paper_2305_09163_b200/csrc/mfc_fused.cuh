@@ -100,12 +100,19 @@ struct NoHook {
     __device__ __forceinline__ void operator()() const {}
 };
 
+// non-uniform spacing: coefficient tables of the tile's first own column (x) and row (y), cf. NuRef (mfc_math.cuh)
+struct NuPlane {
+    const double *tx, *ty;
+    int sx, sy;
+};
+
 // `early` runs at the top of the first FP64-heavy block and `mid` at the top of the second: the caller's loads,
 // cp.async issues and the cons->prim chains of the NEXT plane go there, so that they overlap this plane's
 // arithmetic instead of forming latency-bound phases of their own.
-template <int D, int NF, int TY, int ORDER, class Early = NoHook, class Mid = NoHook>
+template <int D, int NF, int TY, int ORDER, bool NU = false, class Early = NoHook, class Mid = NoHook>
 __device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, const Eos &eos, double cx, double cy,
-                                           double (&acc)[2 * NF + D], Early early = Early(), Mid mid = Mid())
+                                           double (&acc)[2 * NF + D], Early early = Early(), Mid mid = Mid(),
+                                           const NuPlane &nup = NuPlane{nullptr, nullptr, 0, 0})
 {
     using C = FusedCfg<D, NF, TY>;
     using I = Idx<D, NF>;
@@ -136,6 +143,7 @@ __device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, cons
                 int e, r, st;
                 const double *pb;
                 double *dst;
+                NuRef nr{nullptr, 0};                               // (non-uniform: the rim cell's coefficients)
                 if (D >= 2 && u < UY) {
                     const int kind = u / (FTX * NEQ), rem = u - kind * (FTX * NEQ);
                     e = rem / FTX;
@@ -143,6 +151,7 @@ __device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, cons
                     pb = P + e * PPL + (kind == 0 ? HY - 1 : HY + TY) * FPX + NG + r;
                     st = kind == 0 ? FPX : -FPX;
                     dst = (kind == 0 ? B.HyL : B.HyR) + e * FTX + r;
+                    if constexpr (NU) nr = NuRef{nup.ty + (kind == 0 ? -1 : TY), nup.sy};
                 } else {
                     const int v = u - UY, kind = v / (TY * NEQ), rem = v - kind * (TY * NEQ);
                     e = rem / TY;
@@ -150,9 +159,16 @@ __device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, cons
                     pb = P + e * PPL + (r + HY) * FPX + NG + (kind == 0 ? -1 : (kind == 1 ? FTX : 0));
                     st = kind == 0 ? 1 : -1;
                     dst = (kind == 0 ? B.HxL : (kind == 1 ? B.HxR : B.ExR)) + e * TY + r;
+                    if constexpr (NU) nr = NuRef{nup.tx + (kind == 0 ? -1 : (kind == 1 ? FTX : 0)), nup.sx};
                 }
-                double v, unused;
-                reconstruct<ORDER>(pb[0], pb[-st] - pb[-2 * st], pb[0] - pb[-st], pb[st] - pb[0], pb[2 * st] - pb[st], eos.weno_eps4, v, unused);
+                double v, other;
+                if constexpr (NU) {                                 // the coefficients are not mirror images: both sides, one kept
+                    const int sa = st < 0 ? -st : st;
+                    reconstruct<ORDER, true>(pb[0], pb[-sa] - pb[-2 * sa], pb[0] - pb[-sa], pb[sa] - pb[0], pb[2 * sa] - pb[sa], eos.weno_eps4, v, other, nr);
+                    if (st < 0) v = other;
+                } else {
+                    reconstruct<ORDER>(pb[0], pb[-st] - pb[-2 * st], pb[0] - pb[-st], pb[st] - pb[0], pb[2 * st] - pb[st], eos.weno_eps4, v, other);
+                }
                 *dst = v;
             }
         }
@@ -165,7 +181,8 @@ __device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, cons
 #pragma unroll
         for (int e = 0; e < NEQ; ++e) {
             const double *s5 = pc + e * PPL;
-            reconstruct<ORDER>(s5[0], s5[-FPX] - s5[-2 * FPX], s5[0] - s5[-FPX], s5[FPX] - s5[0], s5[2 * FPX] - s5[FPX], eos.weno_eps4, vLy[e], vRy[e]);
+            reconstruct<ORDER, NU>(s5[0], s5[-FPX] - s5[-2 * FPX], s5[0] - s5[-FPX], s5[FPX] - s5[0], s5[2 * FPX] - s5[FPX], eos.weno_eps4, vLy[e], vRy[e],
+                                   NuRef{nup.ty + j, nup.sy});
         }
 #pragma unroll
         for (int e = 0; e < NEQ; ++e) B.X[e * NT + tid] = vRy[e];
@@ -177,7 +194,7 @@ __device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, cons
 #pragma unroll
     for (int e = 0; e < XPRE; ++e) {
         const double *s5 = pc + e * PPL;
-        reconstruct<ORDER>(s5[0], s5[-1] - s5[-2], s5[0] - s5[-1], s5[1] - s5[0], s5[2] - s5[1], eos.weno_eps4, vL[e], vR[e]);
+        reconstruct<ORDER, NU>(s5[0], s5[-1] - s5[-2], s5[0] - s5[-1], s5[1] - s5[0], s5[2] - s5[1], eos.weno_eps4, vL[e], vR[e], NuRef{nup.tx + i, nup.sx});
     }
     __syncthreads();                                                // S1: rim states and y right states are visible
 
@@ -188,7 +205,7 @@ __device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, cons
 #pragma unroll
         for (int e = XPRE; e < NEQ; ++e) {
             const double *s5 = pc + e * PPL;
-            reconstruct<ORDER>(s5[0], s5[-1] - s5[-2], s5[0] - s5[-1], s5[1] - s5[0], s5[2] - s5[1], eos.weno_eps4, vL[e], vR[e]);
+            reconstruct<ORDER, NU>(s5[0], s5[-1] - s5[-2], s5[0] - s5[-1], s5[1] - s5[0], s5[2] - s5[1], eos.weno_eps4, vL[e], vR[e], NuRef{nup.tx + i, nup.sx});
         }
 #pragma unroll
         for (int e = 0; e < NEQ; ++e) {
@@ -280,9 +297,9 @@ __device__ __forceinline__ long long staged_source(const Geo &g, int x0, int y0,
 // ---------------------------------------------------------------------------------------------------------
 // 1D and 2D: one tile per block
 // ---------------------------------------------------------------------------------------------------------
-template <int D, int NF, int TY, int ORDER>
+template <int D, int NF, int TY, int ORDER, bool NU>
 __global__ void __launch_bounds__(FTX *TY, 1)
-    rhs_fused_plane_kernel(Geo g, Eos eos, const double *__restrict__ q, SweepOut o, int ntx)
+    rhs_fused_plane_kernel(typename GeoOf<NU>::type g, Eos eos, const double *__restrict__ q, SweepOut o, int ntx)
 {
     static_assert(D <= 2, "plane kernel");
     using C = FusedCfg<D, NF, TY>;
@@ -314,7 +331,13 @@ __global__ void __launch_bounds__(FTX *TY, 1)
     double acc[NEQ];
 #pragma unroll
     for (int e = 0; e < NEQ; ++e) acc[e] = 0.0;
-    inplane_xy<D, NF, TY, ORDER>(B, eos, o.coef * g.inv_dx[0], D >= 2 ? o.coef * g.inv_dx[1] : 0.0, acc);
+    if constexpr (NU) {   // per-cell widths and coefficient tables (rows of stride g.nus[d], padded past the last cell)
+        const NuPlane nup{g.nu[0] + x0 + NG, D >= 2 ? g.nu[1] + y0 + NG : nullptr, g.nus[0], g.nus[1]};
+        inplane_xy<D, NF, TY, ORDER, true>(B, eos, o.coef * __ldg(nup.tx + i + 27 * nup.sx), D >= 2 ? o.coef * __ldg(nup.ty + j + 27 * nup.sy) : 0.0, acc,
+                                           NoHook(), NoHook(), nup);
+    } else {
+        inplane_xy<D, NF, TY, ORDER>(B, eos, o.coef * g.inv_dx[0], D >= 2 ? o.coef * g.inv_dx[1] : 0.0, acc);
+    }
     if (active) {
 #pragma unroll
         for (int e = 0; e < NEQ; ++e) {
@@ -380,9 +403,9 @@ __device__ __forceinline__ void tmem_store(unsigned a, const double (&v)[TV])
 // ---------------------------------------------------------------------------------------------------------
 // 3D: tile in (x, y), march along z
 // ---------------------------------------------------------------------------------------------------------
-template <int NF, int TY, int ORDER>
+template <int NF, int TY, int ORDER, bool NU>
 __global__ void __launch_bounds__(FTX *TY, 1)
-    rhs_fused_march_kernel(Geo g, Eos eos, const double *__restrict__ q, SweepOut o, int ntx, int nty, int seg)
+    rhs_fused_march_kernel(typename GeoOf<NU>::type g, Eos eos, const double *__restrict__ q, SweepOut o, int ntx, int nty, int seg)
 {
     constexpr int D = 3;
     using C = FusedCfg<D, NF, TY>;
@@ -530,7 +553,16 @@ __global__ void __launch_bounds__(FTX *TY, 1)
         // the three coefficients are re-read from the constant bank every iteration rather than held in registers
         double coef = o.coef;
         asm volatile("" : "+d"(coef));
-        const double cx = coef * g.inv_dx[0], cy = coef * g.inv_dx[1], cz = coef * g.inv_dx[2];
+        NuPlane nup{nullptr, nullptr, 0, 0};
+        if constexpr (NU) nup = NuPlane{g.nu[0] + x0 + NG, g.nu[1] + y0 + NG, g.nus[0], g.nus[1]};
+        double cx, cy, cz;
+        if constexpr (NU) {                                         // the cell's own widths (Eq. 8-9)
+            cx = coef * __ldg(nup.tx + i + 27 * nup.sx);
+            cy = coef * __ldg(nup.ty + j + 27 * nup.sy);
+            cz = coef * __ldg(g.nu[2] + max(ip, 0) + NG + 27 * g.nus[2]);
+        } else {
+            cx = coef * g.inv_dx[0], cy = coef * g.inv_dx[1], cz = coef * g.inv_dx[2];
+        }
 
         double acc[NEQ];
 #pragma unroll
@@ -547,7 +579,7 @@ __global__ void __launch_bounds__(FTX *TY, 1)
                 convert_staged(true, next_inplane ? ip + 1 : -1);
             };
             const InplaneBufs<D, NF, TY> B(P, rim, X, X2, X8);
-            inplane_xy<D, NF, TY, ORDER>(B, eos, cx, cy, acc, early, mid);
+            inplane_xy<D, NF, TY, ORDER, NU>(B, eos, cx, cy, acc, early, mid, nup);
         } else {
             cp_async_wait<1>();
             convert_staged(true, next_inplane ? ip + 1 : -1);
@@ -622,9 +654,11 @@ __global__ void __launch_bounds__(FTX *TY, 1)
                 tmem_load<TV>(tslot(T_PREV), vprev);
 #pragma unroll
                 for (int k = NEQ; k < TV; ++k) vL[k] = 0.0;
+                NuRef nz{nullptr, 0};
+                if constexpr (NU) nz = NuRef{g.nu[2] + c + NG, g.nus[2]};
 #pragma unroll
                 for (int e = 0; e < NEQ; ++e)
-                    reconstruct<ORDER>(rc[e], vb[e] - vprev[e], rc[e] - vb[e], rd[e] - rc[e], wn[e] - rd[e], eos.weno_eps4, vL[e], vR[e]);
+                    reconstruct<ORDER, NU>(rc[e], vb[e] - vprev[e], rc[e] - vb[e], rd[e] - rc[e], wn[e] - rd[e], eos.weno_eps4, vL[e], vR[e], nz);
                 tmem_store<TV>(tslot(T_PARK), vL);
                 if (c >= k0) {
                     double Fm[TV], Fn[TV];                          // previous and new flux; entry NEQ is the face velocity

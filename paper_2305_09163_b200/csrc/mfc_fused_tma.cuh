@@ -76,9 +76,9 @@ struct TmaCfg {
     static_assert(2 * bytes > 227 * 1024, "two resident blocks would deadlock in tcgen05.alloc");
 };
 
-template <int NF, int TY, int ORDER>
+template <int NF, int TY, int ORDER, bool NU>
 __global__ void __launch_bounds__(FTX *TY, 1)
-    rhs_fused_march_tma_kernel(const __grid_constant__ CUtensorMap tm_plane, const __grid_constant__ CUtensorMap tm_col, Geo g, Eos eos,
+    rhs_fused_march_tma_kernel(const __grid_constant__ CUtensorMap tm_plane, const __grid_constant__ CUtensorMap tm_col, typename GeoOf<NU>::type g, Eos eos,
                                SweepOut o, int ntx, int nty, int seg)
 {
     constexpr int D = 3;
@@ -192,7 +192,16 @@ __global__ void __launch_bounds__(FTX *TY, 1)
         double *const Pnext = sm + ((ip + 1) & 1) * T::nPb;
         double coef = o.coef;
         asm volatile("" : "+d"(coef));
-        const double cx = coef * g.inv_dx[0], cy = coef * g.inv_dx[1], cz = coef * g.inv_dx[2];
+        NuPlane nup{nullptr, nullptr, 0, 0};
+        if constexpr (NU) nup = NuPlane{g.nu[0] + x0 + NG, g.nu[1] + y0 + NG, g.nus[0], g.nus[1]};
+        double cx, cy, cz;
+        if constexpr (NU) {                                         // the cell's own widths (Eq. 8-9)
+            cx = coef * __ldg(nup.tx + i + 27 * nup.sx);
+            cy = coef * __ldg(nup.ty + j + 27 * nup.sy);
+            cz = coef * __ldg(g.nu[2] + max(ip, 0) + NG + 27 * g.nus[2]);
+        } else {
+            cx = coef * g.inv_dx[0], cy = coef * g.inv_dx[1], cz = coef * g.inv_dx[2];
+        }
 
         if (tid == 0) {
             if (next_inplane) {
@@ -220,7 +229,7 @@ __global__ void __launch_bounds__(FTX *TY, 1)
                 convert_column(m);
             };
             const InplaneBufs<D, NF, TY> B(Pcur, rim, X, X2, X8);
-            inplane_xy<D, NF, TY, ORDER>(B, eos, cx, cy, acc, early, mid);
+            inplane_xy<D, NF, TY, ORDER, NU>(B, eos, cx, cy, acc, early, mid, nup);
         } else {
             mbar_wait(FULL_SQ, n & 1);
             convert_column(m);
@@ -287,9 +296,11 @@ __global__ void __launch_bounds__(FTX *TY, 1)
                 tmem_load<TV>(tslot(T_PREV), vprev);
 #pragma unroll
                 for (int k = NEQ; k < TV; ++k) vL[k] = 0.0;
+                NuRef nz{nullptr, 0};
+                if constexpr (NU) nz = NuRef{g.nu[2] + c + NG, g.nus[2]};
 #pragma unroll
                 for (int e = 0; e < NEQ; ++e)
-                    reconstruct<ORDER>(rc[e], vb[e] - vprev[e], rc[e] - vb[e], rd[e] - rc[e], wn[e] - rd[e], eos.weno_eps4, vL[e], vR[e]);
+                    reconstruct<ORDER, NU>(rc[e], vb[e] - vprev[e], rc[e] - vb[e], rd[e] - rc[e], wn[e] - rd[e], eos.weno_eps4, vL[e], vR[e], nz);
                 tmem_store<TV>(tslot(T_PARK), vL);
                 if (c >= k0) {
                     double Fm[TV], Fn[TV];

@@ -101,8 +101,8 @@ static bool encode_state_map(CUtensorMap *map, const Geo &g, int neq, const doub
               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-template <int D, int NF, int ORDER>
-static cudaError_t launch_fused(const Geo &g, const Eos &e, const double *q, const SweepOut &o, int segment, int path, cudaStream_t s)
+template <int D, int NF, int ORDER, bool NU>
+static cudaError_t launch_fused_nu(const typename GeoOf<NU>::type &g, const Eos &e, const double *q, const SweepOut &o, int segment, int path, cudaStream_t s)
 {
     constexpr int TY = fused_ty<D, NF>();
     using C = FusedCfg<D, NF, TY>;
@@ -123,22 +123,33 @@ static cudaError_t launch_fused(const Geo &g, const Eos &e, const double *q, con
                             (o.nbase == 0 || o.qs == q);
         CUtensorMap tm_plane, tm_col;
         if (tma_ok && encode_state_map(&tm_plane, g, C::NEQ, q, FPX, C::PY) && encode_state_map(&tm_col, g, C::NEQ, q, T::CW, TY)) {
-            if ((st = MFC_OPTIN_SHARED((rhs_fused_march_tma_kernel<NF, TY, ORDER>), T::bytes)) != cudaSuccess) return st;
-            rhs_fused_march_tma_kernel<NF, TY, ORDER><<<blocks, C::NT, T::bytes, s>>>(tm_plane, tm_col, g, e, o, ntx, nty, seg);
+            if ((st = MFC_OPTIN_SHARED((rhs_fused_march_tma_kernel<NF, TY, ORDER, NU>), T::bytes)) != cudaSuccess) return st;
+            rhs_fused_march_tma_kernel<NF, TY, ORDER, NU><<<blocks, C::NT, T::bytes, s>>>(tm_plane, tm_col, g, e, o, ntx, nty, seg);
         } else {
             if (path == MFC_PATH_TMA) return cudaErrorInvalidValue;
-            if ((st = MFC_OPTIN_SHARED((rhs_fused_march_kernel<NF, TY, ORDER>), C::bytes)) != cudaSuccess) return st;
-            rhs_fused_march_kernel<NF, TY, ORDER><<<blocks, C::NT, C::bytes, s>>>(g, e, q, o, ntx, nty, seg);
+            if ((st = MFC_OPTIN_SHARED((rhs_fused_march_kernel<NF, TY, ORDER, NU>), C::bytes)) != cudaSuccess) return st;
+            rhs_fused_march_kernel<NF, TY, ORDER, NU><<<blocks, C::NT, C::bytes, s>>>(g, e, q, o, ntx, nty, seg);
         }
     } else {
-        if ((st = MFC_OPTIN_SHARED((rhs_fused_plane_kernel<D, NF, TY, ORDER>), C::bytes)) != cudaSuccess) return st;
-        rhs_fused_plane_kernel<D, NF, TY, ORDER><<<(unsigned)((long long)ntx * nty), C::NT, C::bytes, s>>>(g, e, q, o, ntx);
+        if ((st = MFC_OPTIN_SHARED((rhs_fused_plane_kernel<D, NF, TY, ORDER, NU>), C::bytes)) != cudaSuccess) return st;
+        rhs_fused_plane_kernel<D, NF, TY, ORDER, NU><<<(unsigned)((long long)ntx * nty), C::NT, C::bytes, s>>>(g, e, q, o, ntx);
     }
     return cudaSuccess;
 }
 
+// non-uniform spacing (Geo::nonuniform) selects the table-driven instantiation; it exists for WENO5 only
+template <int D, int NF, int ORDER>
+static cudaError_t launch_fused(const GeoNu &g, const Eos &e, const double *q, const SweepOut &o, int segment, int path, cudaStream_t s)
+{
+    if (g.nu[0]) {
+        if constexpr (ORDER == 5) return launch_fused_nu<D, NF, ORDER, true>(g, e, q, o, segment, path, s);
+        else return cudaErrorInvalidValue;
+    }
+    return launch_fused_nu<D, NF, ORDER, false>(g, e, q, o, segment, path, s);
+}
+
 template <int D, int NF>
-static cudaError_t launch_fused_order(int order, const Geo &g, const Eos &e, const double *q, const SweepOut &o, int segment, int path,
+static cudaError_t launch_fused_order(int order, const GeoNu &g, const Eos &e, const double *q, const SweepOut &o, int segment, int path,
                                       cudaStream_t s)
 {
     cudaError_t st = cudaSuccess;
@@ -146,7 +157,7 @@ static cudaError_t launch_fused_order(int order, const Geo &g, const Eos &e, con
     return st;
 }
 
-cudaError_t MFC_CAT(launch_rhs_d, MFC_D)(int nf, int order, const Geo &g, const Eos &e, const double *q, const SweepOut &o,
+cudaError_t MFC_CAT(launch_rhs_d, MFC_D)(int nf, int order, const GeoNu &g, const Eos &e, const double *q, const SweepOut &o,
                                          int segment, int path, cudaStream_t s)
 {
     constexpr int D = MFC_D;
@@ -155,37 +166,43 @@ cudaError_t MFC_CAT(launch_rhs_d, MFC_D)(int nf, int order, const Geo &g, const 
     return err != cudaSuccess ? err : cudaGetLastError();
 }
 
-cudaError_t MFC_CAT(launch_cfl_d, MFC_D)(int nf, const Geo &g, const Eos &e, const double *q, unsigned long long *min_bits,
+cudaError_t MFC_CAT(launch_cfl_d, MFC_D)(int nf, const GeoNu &g, const Eos &e, const double *q, unsigned long long *min_bits,
                                          cudaStream_t s)
 {
     constexpr int D = MFC_D;
     const long long ncell = (long long)g.n[0] * g.n[1] * g.n[2];
     long long want = (ncell + 255) / 256;
     const unsigned blocks = (unsigned)(want < 148 * 16 ? (want < 1 ? 1 : want) : 148 * 16);
-    MFC_FOR_NF(nf, (cfl_kernel<D, NF><<<blocks, 256, 0, s>>>(g, e, q, min_bits)))
+    if (g.nu[0]) { MFC_FOR_NF(nf, (cfl_kernel<D, NF, true><<<blocks, 256, 0, s>>>(g, e, q, min_bits))) }
+    else { MFC_FOR_NF(nf, (cfl_kernel<D, NF, false><<<blocks, 256, 0, s>>>((const Geo &)g, e, q, min_bits))) }
     return cudaGetLastError();
 }
 
 template <int D, int NF, int DIR>
 static cudaError_t launch_line_t(int order, const Eos &e, int n, const double *w, double *vL, double *vR, double *F, double *uf,
-                                 cudaStream_t s)
+                                 const double *nu, int nus, cudaStream_t s)
 {
-    MFC_FOR_ORDER(order, (line_weno_kernel<D, NF, DIR, ORDER><<<(n + 2 + 127) / 128, 128, 0, s>>>(e, n, w, vL, vR)))
+    if (nu) {
+        if (order != 5) return cudaErrorInvalidValue;
+        line_weno_kernel<D, NF, DIR, 5, true><<<(n + 2 + 127) / 128, 128, 0, s>>>(e, n, w, vL, vR, nu, nus);
+    } else {
+        MFC_FOR_ORDER(order, (line_weno_kernel<D, NF, DIR, ORDER, false><<<(n + 2 + 127) / 128, 128, 0, s>>>(e, n, w, vL, vR, nullptr, 0)))
+    }
     line_hllc_kernel<D, NF, DIR><<<(n + 1 + 127) / 128, 128, 0, s>>>(e, n, vL, vR, F, uf);
     return cudaSuccess;
 }
 
 cudaError_t MFC_CAT(launch_line_d, MFC_D)(int nf, int order, int dir, const Eos &e, int n, const double *w, double *vL, double *vR,
-                                          double *F, double *uf, cudaStream_t s)
+                                          double *F, double *uf, const double *nu, int nus, cudaStream_t s)
 {
     constexpr int D = MFC_D;
     if (dir < 0 || dir >= D) return cudaErrorInvalidValue;
-    if (dir == 0) { MFC_FOR_NF(nf, (launch_line_t<D, NF, 0>(order, e, n, w, vL, vR, F, uf, s))) }
+    if (dir == 0) { MFC_FOR_NF(nf, (launch_line_t<D, NF, 0>(order, e, n, w, vL, vR, F, uf, nu, nus, s))) }
 #if MFC_D >= 2
-    else if (dir == 1) { MFC_FOR_NF(nf, (launch_line_t<D, NF, 1>(order, e, n, w, vL, vR, F, uf, s))) }
+    else if (dir == 1) { MFC_FOR_NF(nf, (launch_line_t<D, NF, 1>(order, e, n, w, vL, vR, F, uf, nu, nus, s))) }
 #endif
 #if MFC_D >= 3
-    else if (dir == 2) { MFC_FOR_NF(nf, (launch_line_t<D, NF, 2>(order, e, n, w, vL, vR, F, uf, s))) }
+    else if (dir == 2) { MFC_FOR_NF(nf, (launch_line_t<D, NF, 2>(order, e, n, w, vL, vR, F, uf, nu, nus, s))) }
 #endif
     return cudaGetLastError();
 }

@@ -37,7 +37,7 @@ __global__ void __launch_bounds__(256) prim_kernel(Geo g, Eos eos, const double 
 // per cell against about 70 FP64 instructions).
 // ---------------------------------------------------------------------------------------------------------
 template <int D, int NF>
-__device__ __forceinline__ double cell_signal_speed(const Geo &g, const Eos &eos, const double (&qc)[2 * NF + D])
+__device__ __forceinline__ double cell_signal_speed(const double (&inv_dx)[3], const Eos &eos, const double (&qc)[2 * NF + D])
 {
     using I = Idx<D, NF>;
     double wc[I::NEQ];
@@ -52,30 +52,39 @@ __device__ __forceinline__ double cell_signal_speed(const Geo &g, const Eos &eos
     const double cs = fabs(num) * rsqrt_fast(num * (G * rho));       // frozen mixture sound speed (reading B2)
     double s = 0.0;
 #pragma unroll
-    for (int d = 0; d < D; ++d) s = fmax(s, g.inv_dx[d] * (fabs(wc[I::U + d]) + cs));
+    for (int d = 0; d < D; ++d) s = fmax(s, inv_dx[d] * (fabs(wc[I::U + d]) + cs));
     return s;
 }
 
-template <int D, int NF>
-__global__ void __launch_bounds__(256) cfl_kernel(Geo g, Eos eos, const double *__restrict__ q, unsigned long long *max_bits)
+template <int D, int NF, bool NU>
+__global__ void __launch_bounds__(256) cfl_kernel(typename GeoOf<NU>::type g, Eos eos, const double *__restrict__ q, unsigned long long *max_bits)
 {
     using I = Idx<D, NF>;
     const long long ncell = (long long)g.n[0] * g.n[1] * g.n[2];
     const long long stride = (long long)gridDim.x * blockDim.x;
-    auto cell_of = [&](long long f) -> long long {
+    // cell f of the interior (x fastest): offset in the padded array and the inverse widths of the cell (Eq. 8)
+    auto cell_of = [&](long long f, double (&inv)[3]) -> long long {
         const int i = (int)(f % g.n[0]);
         const long long r = f / g.n[0];
         const int j = (int)(r % g.n[1]), k = (int)(r / g.n[1]);
+        if constexpr (NU) {
+            inv[0] = __ldg(g.nu[0] + i + NG + 27 * g.nus[0]);
+            inv[1] = D > 1 ? __ldg(g.nu[1] + j + NG + 27 * g.nus[1]) : 1.0;
+            inv[2] = D > 2 ? __ldg(g.nu[2] + k + NG + 27 * g.nus[2]) : 1.0;
+        } else {
+            inv[0] = g.inv_dx[0]; inv[1] = g.inv_dx[1]; inv[2] = g.inv_dx[2];
+        }
         return (long long)(k + g.g[2]) * g.sz + (long long)(j + g.g[1]) * g.sy + (i + NG);
     };
     double best = 0.0;
     for (long long f = (long long)blockIdx.x * blockDim.x + threadIdx.x; f < ncell; f += 2 * stride) {
         const bool two = f + stride < ncell;
-        const long long c0 = cell_of(f), c1 = cell_of(two ? f + stride : f);
+        double i0[3], i1[3];
+        const long long c0 = cell_of(f, i0), c1 = cell_of(two ? f + stride : f, i1);
         double q0[I::NEQ], q1[I::NEQ];
 #pragma unroll
         for (int e = 0; e < I::NEQ; ++e) { q0[e] = __ldg(q + (long long)e * g.cells + c0); q1[e] = __ldg(q + (long long)e * g.cells + c1); }
-        best = fmax(best, fmax(cell_signal_speed<D, NF>(g, eos, q0), cell_signal_speed<D, NF>(g, eos, q1)));
+        best = fmax(best, fmax(cell_signal_speed<D, NF>(i0, eos, q0), cell_signal_speed<D, NF>(i1, eos, q1)));
     }
 #pragma unroll
     for (int off = 16; off > 0; off >>= 1) best = fmax(best, __shfl_xor_sync(0xffffffffu, best, off));
@@ -91,8 +100,8 @@ __global__ void __launch_bounds__(256) cfl_kernel(Geo g, Eos eos, const double *
 // ---------------------------------------------------------------------------------------------------------
 // a2 + a3 on one line of primitives (stage parity): same weno5 / hllc as the sweeps, one thread per cell.
 // ---------------------------------------------------------------------------------------------------------
-template <int D, int NF, int DIR, int ORDER>
-__global__ void line_weno_kernel(Eos eos, int n, const double *__restrict__ w, double *vL, double *vR)
+template <int D, int NF, int DIR, int ORDER, bool NU>
+__global__ void line_weno_kernel(Eos eos, int n, const double *__restrict__ w, double *vL, double *vR, const double *nu, int nus)
 {
     using I = Idx<D, NF>;
     const int t = blockIdx.x * blockDim.x + threadIdx.x;   // cell t - 1
@@ -102,7 +111,7 @@ __global__ void line_weno_kernel(Eos eos, int n, const double *__restrict__ w, d
     for (int e = 0; e < I::NEQ; ++e) {
         const double *p = w + (long long)e * np + (t - 1 + NG);
         double l, r;
-        reconstruct<ORDER>(p[0], p[-1] - p[-2], p[0] - p[-1], p[1] - p[0], p[2] - p[1], eos.weno_eps4, l, r);
+        reconstruct<ORDER, NU>(p[0], p[-1] - p[-2], p[0] - p[-1], p[1] - p[0], p[2] - p[1], eos.weno_eps4, l, r, NuRef{NU ? nu + t - 1 + NG : nullptr, nus});
         vL[(long long)e * (n + 2) + t] = l;
         vR[(long long)e * (n + 2) + t] = r;
     }

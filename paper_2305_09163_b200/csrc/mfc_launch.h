@@ -21,6 +21,19 @@ struct Geo {
     int sms;             // multiprocessors of the device (persistent grids are sized from it)
 };
 
+// non-uniform Cartesian spacing (Listing 1): per direction a device table [NU_NC][nus[d]] of the per-index
+// WENO5 coefficients (beta_coef, poly_coef, d_cb of Listing 1) and the inverse cell width.  Only the table-driven
+// instantiations (template flag NU) take this struct; the uniform ones take a plain Geo, so that their parameters and
+// code are untouched by the feature.
+struct GeoNu : Geo {
+    const double *nu[3];
+    int nus[3];          // row stride of nu[d] (p[d] plus padding, so that ragged tiles read defined entries)
+};
+template <bool NU> struct GeoOf { typedef Geo type; };
+template <> struct GeoOf<true> { typedef GeoNu type; };
+
+constexpr int NU_NC = 28;    // 9 beta_coef + 6 poly_coef (left) + 6 poly_coef (right) + 3 + 3 ideal weights + 1 / width
+
 // stiffened-gas tables, PAPER.md:54-58 (Eq. 1), alpha-weighted mixture (reading B2)
 struct Eos {
     // as given / as the definition divides by: used by the cons->prim kernel, which evaluates the
@@ -51,24 +64,25 @@ cudaError_t launch_prim(int ndim, int nf, const Geo &g, const Eos &e, const doub
 // staging path of the 3D kernel: AUTO = TMA boxes where the layout allows them (even padded extent in x, 16-byte
 // aligned base), else per-thread cp.async; the other two force one of them (TMA fails if the layout does not allow it)
 enum { MFC_PATH_AUTO = 0, MFC_PATH_TMA = 1, MFC_PATH_LDGSTS = 2 };
-cudaError_t launch_rhs(int ndim, int nf, int order, const Geo &g, const Eos &e, const double *q, const SweepOut &o, int segment,
+// g.nu[0] != nullptr selects the table-driven (non-uniform) instantiations
+cudaError_t launch_rhs(int ndim, int nf, int order, const GeoNu &g, const Eos &e, const double *q, const SweepOut &o, int segment,
                        int path, cudaStream_t s);
 cudaError_t launch_ghost_fill(const Geo &g, int neq, double *q, cudaStream_t s);
-cudaError_t launch_cfl(int ndim, int nf, const Geo &g, const Eos &e, const double *q, unsigned long long *min_bits,
+cudaError_t launch_cfl(int ndim, int nf, const GeoNu &g, const Eos &e, const double *q, unsigned long long *min_bits,
                        cudaStream_t s);
 cudaError_t launch_eos_seed(const double *gm1_dev, double *ygm1_dev, int n, cudaStream_t s);
 cudaError_t launch_line(int ndim, int nf, int order, int dir, const Eos &e, int n, const double *w, double *vL, double *vR,
-                        double *F, double *uf, cudaStream_t s);
+                        double *F, double *uf, const double *nu, int nus, cudaStream_t s);
 
 // per-dimension implementations
 #define MFC_DECL_DIM(D)                                                                                               \
     cudaError_t launch_prim_d##D(int nf, const Geo &g, const Eos &e, const double *q, double *w, cudaStream_t s);     \
-    cudaError_t launch_rhs_d##D(int nf, int order, const Geo &g, const Eos &e, const double *q, const SweepOut &o, int segment,  \
+    cudaError_t launch_rhs_d##D(int nf, int order, const GeoNu &g, const Eos &e, const double *q, const SweepOut &o, int segment,  \
                                 int path, cudaStream_t s);                                                            \
-    cudaError_t launch_cfl_d##D(int nf, const Geo &g, const Eos &e, const double *q, unsigned long long *min_bits,    \
+    cudaError_t launch_cfl_d##D(int nf, const GeoNu &g, const Eos &e, const double *q, unsigned long long *min_bits,  \
                                 cudaStream_t s);                                                                      \
     cudaError_t launch_line_d##D(int nf, int order, int dir, const Eos &e, int n, const double *w, double *vL, double *vR,       \
-                                 double *F, double *uf, cudaStream_t s);
+                                 double *F, double *uf, const double *nu, int nus, cudaStream_t s);
 MFC_DECL_DIM(1)
 MFC_DECL_DIM(2)
 MFC_DECL_DIM(3)

@@ -101,7 +101,8 @@ def rhs_floors(prob, orc, q: np.ndarray) -> np.ndarray:
     it = prob.interior()
     w = orc.cons_to_prim(q)[it]
     nf, D = prob.nf, prob.ndim
-    dxmin, dxmax = min(prob.dx[:D]), max(prob.dx[:D])
+    dxmin = min(float(np.min(prob.widths(d))) for d in range(D))
+    dxmax = max(float(np.max(prob.widths(d))) for d in range(D))
     lam = dxmax / orc.cfl_dt(q, 1.0)                           # >= max_d max_cells (|u_d| + c)
     rho = w[:nf].sum(axis=0)
     umax = max(float(np.max(np.abs(w[nf + d]))) for d in range(D))

@@ -341,6 +341,104 @@ def test_rhs_parity_cfg4_reduced():
 
 
 # ---------------------------------------------------------------------------------------------
+# Non-uniform Cartesian spacing (Listing 1, Eq. 15): same bars on stretched grids
+# ---------------------------------------------------------------------------------------------
+NU_CASES = [(1, 1, (1201,)), (1, 2, (600,)), (2, 2, (300, 45)), (2, 3, (131, 46)), (3, 1, (66, 29, 41)), (3, 2, (67, 29, 41)),
+            (3, 2, (70, 30, 40)), (3, 3, (40, 29, 33))]
+
+
+@pytest.mark.parametrize("ndim,nf,n", NU_CASES)
+@pytest.mark.parametrize("periodic", [True, False])
+def test_rhs_parity_stretched_grid(ndim, nf, n, periodic):
+    prob, q = wl.random_state(ndim, n, nf, seed=400 + 10 * ndim + nf, periodic=periodic)
+    prob = wl.with_stretched_grid(prob)
+    check_rhs(prob, q, march_segment=8)
+    with Gpu(prob) as g1, Gpu(__import__("dataclasses").replace(prob, edges=None)) as g0:     # the grid is really in use
+        it = prob.interior()
+        assert not np.allclose(g1.rhs(q)[it], g0.rhs(q)[it], rtol=1e-3)
+
+
+@pytest.mark.parametrize("staging", [B.MFC_STAGING_TMA, B.MFC_STAGING_CPASYNC])
+def test_rhs_parity_stretched_grid_both_staging_paths(staging):
+    prob, q = wl.random_state(3, (70, 29, 41), 2, seed=433, periodic=False)
+    check_rhs(wl.with_stretched_grid(prob), q, march_segment=8, staging=staging)
+
+
+@pytest.mark.parametrize("dims", [(0,), (1,), (2,), (0, 2)])
+def test_rhs_parity_grid_stretched_in_some_dimensions_only(dims):
+    prob, q = wl.random_state(3, (40, 29, 33), 2, seed=440 + len(dims) + dims[0], periodic=True)
+    check_rhs(wl.with_stretched_grid(prob, dims=dims), q, march_segment=8)
+
+
+def test_uniform_edges_reproduce_the_uniform_kernel_to_round_off():
+    import dataclasses
+    prob, q = wl.random_state(3, (40, 29, 33), 2, seed=450, periodic=False)
+    pe = dataclasses.replace(prob, edges=tuple(np.linspace(prob.lo[d], prob.hi[d], prob.n[d] + 1) for d in range(3)))
+    it = prob.interior()
+    with Gpu(prob) as g0, Gpu(pe) as g1:
+        a, b = g0.rhs(q)[it], g1.rhs(q)[it]
+    for k in range(prob.neq):
+        assert np.max(np.abs(a[k] - b[k])) <= 1e-11 * np.max(np.abs(a[k]))
+
+
+@pytest.mark.parametrize("ndim,nf,n", [(1, 2, (600,)), (2, 2, (130, 45)), (3, 2, (40, 29, 33)), (3, 3, (40, 30, 33))])
+@pytest.mark.parametrize("rough", [False, True])
+def test_rk3_parity_stretched_grid(ndim, nf, n, rough):
+    prob, q = wl.random_state(ndim, n, nf, seed=460 + ndim + nf, periodic=(nf != 2), rough=rough)
+    check_rk(wl.with_stretched_grid(prob), q, march_segment=8)
+
+
+def test_rhs_and_rk3_parity_cfg2_stretched():
+    """The shock-bubble workload on the Eq. 15 grid (same per-cell data on stretched cells), default launch configuration."""
+    prob, q = wl.cfg2(n=64)
+    prob = wl.with_stretched_grid(prob)
+    check_rhs(prob, q)
+    check_rk(prob, q)
+
+
+def test_cfl_dt_parity_stretched_grid():
+    for ndim, n in [(1, (301,)), (2, (65, 33)), (3, (40, 29, 33))]:
+        prob, q = wl.random_state(ndim, n, 2, seed=470 + ndim, periodic=True)
+        prob = wl.with_stretched_grid(prob)
+        ref = oracle.Oracle(prob).cfl_dt(q, prob.cfl)
+        with Gpu(prob) as g:
+            got = g.cfl_dt(q)
+        assert abs(got - ref) <= 1e-13 * ref
+
+
+def test_line_states_and_fluxes_stretched_grid():
+    n = 777
+    prob, _ = wl.random_state(2, (8, n), 2, seed=1)
+    prob = wl.with_stretched_grid(prob)
+    orc = oracle.Oracle(prob)
+    w = random_prim_line(prob, n, np.random.default_rng(480), False)
+    rL, rR, rF, ru = orc.line(1, w)
+    with Gpu(prob) as g:
+        gL, gR, gF, gu = g.line(1, w)
+        with pytest.raises(B.MfcError):          # a line of another length has no coefficient table
+            g.line(0, w)
+    for e in range(prob.neq):
+        s = np.max(np.abs(w[e])) + 1e-300
+        assert np.max(np.abs(gL[e] - rL[e])) <= 1e-13 * s and np.max(np.abs(gR[e] - rR[e])) <= 1e-13 * s
+        assert np.max(np.abs(gF[e] - rF[e])) <= 1e-11 * (np.max(np.abs(rF[e])) + 1e-300)
+
+
+def test_nonuniform_grid_needs_weno5_and_increasing_edges():
+    import dataclasses
+    prob, q = wl.random_state(2, (20, 12), 2, seed=1)
+    ps = wl.with_stretched_grid(prob)
+    with pytest.raises(B.MfcError) as ei:
+        Gpu(dataclasses.replace(ps, weno_order=3))
+    assert ei.value.code == B.MFC_EUNSUPPORTED
+    bad = list(ps.edges)
+    bad[0] = np.array(bad[0])
+    bad[0][5] = bad[0][3]
+    with pytest.raises(B.MfcError) as ei:
+        Gpu(dataclasses.replace(ps, edges=tuple(bad)))
+    assert ei.value.code == B.MFC_EINVAL
+
+
+# ---------------------------------------------------------------------------------------------
 # full sizes in the launch configuration bench.py times: sampled sub-boxes the oracle can compute
 # (L at a cell depends on the 6 axis neighbours up to distance 3 only) plus size-independent properties
 # ---------------------------------------------------------------------------------------------
