@@ -49,7 +49,8 @@ typedef enum {
     MFC_EUNSUPPORTED = -2, /* (ndim, n_fluids) outside the compiled template set; kapila with n_fluids != 2; non-uniform
                               spacing with weno_order != 5 or with a non-positive ideal weight */
     MFC_ECUDA = -3,        /* CUDA runtime error (sticky); no device */
-    MFC_ENOMEM = -4        /* device or host allocation failed */
+    MFC_ENOMEM = -4,       /* device or host allocation failed */
+    MFC_ENONFINITE = -5    /* mfc_advance_host: the CFL time step of the current state is NaN, infinite or zero */
 } mfc_status;
 
 /* Cartesian grid, PAPER.md:105-124 (Eq. 6-9).  Uniform by default: dx_d = (hi_d - lo_d) / n_d.
@@ -120,13 +121,17 @@ int mfc_rhs(mfc_ctx *ctx, double *q_dev, double *rhs_dev, void *stream);
 int mfc_rk3_step(mfc_ctx *ctx, double *q_dev, double dt, void *stream);
 
 /* CFL-restricted time step: dt = cfl * min over interior cells and directions of
- * dx_d / (|u_d| + c), c the frozen mixture sound speed.  Synchronises `stream`; writes one host double. */
+ * dx_d / (|u_d| + c), c the frozen mixture sound speed (dx_d the cell's own width).  Synchronises `stream`; writes one
+ * host double.  A cell whose signal speed is not finite (NaN input, negative c^2, zero density) makes the result NaN:
+ * the reduction keeps NaN, it does not drop it; the call still returns MFC_OK. */
 int mfc_cfl_dt(mfc_ctx *ctx, const double *q_dev, double *dt_host, void *stream);
 
 /* Whole path from HOST memory: copies q_host to the device, takes nsteps RK3 steps (each with
  * dt = dt_fixed if dt_fixed > 0, else the CFL step of the current state), copies the state back into
  * q_host and synchronises.  t_host (may be NULL) receives the sum of the steps taken.
- * q_host: `elems` doubles in the layout above; pinned memory makes the copies asynchronous. */
+ * q_host: `elems` doubles in the layout above; pinned memory makes the copies asynchronous.
+ * With dt_fixed <= 0, a step whose CFL time step is not finite and positive is not taken: MFC_ENONFINITE is returned
+ * and q_host is left untouched. */
 int mfc_advance_host(mfc_ctx *ctx, double *q_host, int nsteps, double dt_fixed, double *t_host, void *stream);
 
 /* ---- stage outputs, for parity tests of the individual steps of the path ---- */

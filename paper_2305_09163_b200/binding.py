@@ -14,7 +14,7 @@ _HERE = Path(__file__).resolve().parent
 LIB_PATH = _HERE / "libmfc_b200.so"
 
 MFC_NG = 3
-MFC_OK, MFC_EINVAL, MFC_EUNSUPPORTED, MFC_ECUDA, MFC_ENOMEM = 0, -1, -2, -3, -4
+MFC_OK, MFC_EINVAL, MFC_EUNSUPPORTED, MFC_ECUDA, MFC_ENOMEM, MFC_ENONFINITE = 0, -1, -2, -3, -4, -5
 MFC_BC_PERIODIC, MFC_BC_EXTRAP = 0, 1
 MFC_K_RHS, MFC_K_CFL, MFC_K_PRIM, MFC_K_GHOST, MFC_K_COUNT = 0, 1, 2, 3, 4
 KERNEL_NAMES = {MFC_K_RHS: "rhs_fused", MFC_K_CFL: "cfl", MFC_K_PRIM: "prim", MFC_K_GHOST: "ghost_fill"}

@@ -397,6 +397,7 @@ const char *mfc_strerror(int code)
         case MFC_EUNSUPPORTED: return "(ndim, n_fluids) not in the compiled template set";
         case MFC_ECUDA: return "CUDA runtime error";
         case MFC_ENOMEM: return "out of memory";
+        case MFC_ENONFINITE: return "the state is not admissible: the CFL time step is not finite";
     }
     return "unknown error";
 }
@@ -605,6 +606,7 @@ int mfc_advance_host(mfc_ctx *c, double *q_host, int nsteps, double dt_fixed, do
         if (!(dt_fixed > 0.0)) {
             const int st = cfl_dt(c, c->q_own, &dt, s);
             if (st) return st;
+            if (!std::isfinite(dt) || !(dt > 0.0)) return MFC_ENONFINITE;    // inadmissible state: do not step on
         }
         const int st = rk3(c, c->q_own, dt, s);
         if (st) return st;

@@ -50,10 +50,14 @@ __device__ __forceinline__ double cell_signal_speed(const double (&inv_dx)[3], c
     for (int e = 0; e < I::NA; ++e) { G = fma(wc[I::A + e], eos.dG[e], G); P = fma(wc[I::A + e], eos.dP[e], P); }
     const double num = fma(G, wc[I::E], P) + wc[I::E];               // (Gamma + 1) p + Pi
     const double cs = fabs(num) * rsqrt_fast(num * (G * rho));       // frozen mixture sound speed (reading B2)
-    double s = 0.0;
+    double s = 0.0, sum = 0.0;
 #pragma unroll
-    for (int d = 0; d < D; ++d) s = fmax(s, inv_dx[d] * (fabs(wc[I::U + d]) + cs));
-    return s;
+    for (int d = 0; d < D; ++d) {
+        const double sd = inv_dx[d] * (fabs(wc[I::U + d]) + cs);
+        s = fmax(s, sd);
+        sum += sd;                                                   // NaN if any direction is (fmax would drop it)
+    }
+    return sum == sum ? s : sum;
 }
 
 template <int D, int NF, bool NU>
@@ -76,7 +80,13 @@ __global__ void __launch_bounds__(256) cfl_kernel(typename GeoOf<NU>::type g, Eo
         }
         return (long long)(k + g.g[2]) * g.sz + (long long)(j + g.g[1]) * g.sy + (i + NG);
     };
-    double best = 0.0;
+    // the maximum is taken on the BIT PATTERNS: non-negative doubles order like unsigned integers, and so do +inf and NaN
+    // above them -- a non-finite signal speed (inadmissible state: negative c^2, rho = 0, NaN input) is not dropped the way
+    // fmax would drop it, it wins the reduction and the host sees dt = NaN (mfc.h: inadmissible states propagate as NaN)
+    unsigned long long best = 0ull;
+    auto bits = [](double s) -> unsigned long long {
+        return (unsigned long long)__double_as_longlong(s == s ? s : __longlong_as_double(0x7ff8000000000000ll));
+    };
     for (long long f = (long long)blockIdx.x * blockDim.x + threadIdx.x; f < ncell; f += 2 * stride) {
         const bool two = f + stride < ncell;
         double i0[3], i1[3];
@@ -84,16 +94,17 @@ __global__ void __launch_bounds__(256) cfl_kernel(typename GeoOf<NU>::type g, Eo
         double q0[I::NEQ], q1[I::NEQ];
 #pragma unroll
         for (int e = 0; e < I::NEQ; ++e) { q0[e] = __ldg(q + (long long)e * g.cells + c0); q1[e] = __ldg(q + (long long)e * g.cells + c1); }
-        best = fmax(best, fmax(cell_signal_speed<D, NF>(i0, eos, q0), cell_signal_speed<D, NF>(i1, eos, q1)));
+        const unsigned long long b0 = bits(cell_signal_speed<D, NF>(i0, eos, q0)), b1 = bits(cell_signal_speed<D, NF>(i1, eos, q1));
+        best = max(best, max(b0, b1));
     }
 #pragma unroll
-    for (int off = 16; off > 0; off >>= 1) best = fmax(best, __shfl_xor_sync(0xffffffffu, best, off));
-    __shared__ double red[8];
+    for (int off = 16; off > 0; off >>= 1) best = max(best, __shfl_xor_sync(0xffffffffu, best, off));
+    __shared__ unsigned long long red[8];
     if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = best;
     __syncthreads();
     if (threadIdx.x == 0) {
-        for (int wi = 1; wi < (int)(blockDim.x >> 5); ++wi) best = fmax(best, red[wi]);
-        atomicMax(max_bits, (unsigned long long)__double_as_longlong(best));
+        for (int wi = 1; wi < (int)(blockDim.x >> 5); ++wi) best = max(best, red[wi]);
+        atomicMax(max_bits, best);
     }
 }
 

@@ -616,6 +616,53 @@ def test_cfl_dt_parity_cfg3():
     assert abs(got - ref) <= 1e-13 * ref
 
 
+def test_cfl_dt_propagates_nan_and_advance_host_stops():
+    """An inadmissible cell (NaN energy; negative c^2) must not be dropped by the max-reduction: dt is NaN, and
+    mfc_advance_host refuses to step on."""
+    prob, q = wl.random_state(3, (20, 12, 9), 2, seed=4, periodic=True)
+    it = prob.interior()
+    for poison in ("nan", "negative_c2"):
+        qb = q.copy()
+        if poison == "nan":
+            qb[it][prob.nf + prob.ndim][3, 5, 7] = np.nan
+        else:
+            qb[it][prob.nf + prob.ndim][3, 5, 7] = -1.0e12          # p so negative that (Gamma + 1) p + Pi < 0
+        with Gpu(prob) as g:
+            assert np.isnan(g.cfl_dt(qb))
+            qh = g.torch.from_numpy(qb.copy()).pin_memory()
+            with pytest.raises(B.MfcError) as ei:
+                B.mfc_advance_host(g.ctx, qh.data_ptr(), 1, 0.0, g.stream)
+            assert ei.value.code == B.MFC_ENONFINITE
+            assert np.array_equal(qh.numpy(), qb, equal_nan=True)
+
+
+def test_step_runs_beside_a_tensor_core_kernel_on_another_stream():
+    """The 3D kernel takes all 512 TMEM columns of a multiprocessor (mfc.h "Tensor memory"); a tcgen05 GEMM on another
+    stream is serialised against it by the hardware allocator, in either order, without deadlock and without changing a bit."""
+    prob, q = wl.random_state(3, (96, 72, 64), 2, seed=31, periodic=False, rough=False)
+    orc = oracle.Oracle(prob)
+    dts = [0.5 * orc.cfl_dt(q.copy(), prob.cfl)] * 4
+    with Gpu(prob) as g:
+        torch = g.torch
+        alone = g.rk3(q, dts)
+        a = torch.randn(4096, 4096, device=g.dev, dtype=torch.bfloat16)
+        b = torch.randn(4096, 4096, device=g.dev, dtype=torch.bfloat16)
+        side = torch.cuda.Stream()
+        qd = g.to_dev(q)
+        torch.cuda.synchronize()
+        with torch.cuda.stream(side):
+            for _ in range(40):
+                c = a @ b
+        for dt in dts:
+            B.mfc_rk3_step(g.ctx, qd.data_ptr(), float(dt), g.stream)
+            with torch.cuda.stream(side):
+                for _ in range(10):
+                    c = a @ b
+        torch.cuda.synchronize()
+        assert torch.isfinite(c.float()).all()
+        assert np.array_equal(qd.cpu().numpy()[prob.interior()], alone[prob.interior()])
+
+
 # ---------------------------------------------------------------------------------------------
 # host-buffer entry point and measurement hooks
 # ---------------------------------------------------------------------------------------------
