@@ -40,18 +40,25 @@ def measured_peaks():
     return 6650.0, "fallback"
 
 
+TRAFFIC_CSV = os.path.join("profiles", "r02_dram_traffic.csv")
+
+
 def ncu_traffic(workload: str, kernel: str):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` on `workload`, from the committed ncu
-    capture (profiles/r01_dram_traffic.csv names the report and the command); None when no capture is recorded."""
-    path = os.path.join(ROOT, "profiles", "r01_dram_traffic.csv")
+    """(dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` on `workload`, provenance) from the committed
+    ncu capture (profiles/r02_dram_traffic.csv: one `ncu --set full` run, its command and the commit it profiled are in
+    the file).  It is RECORDED, not measured in this run: the provenance string says which commit it belongs to.
+    (None, None) when no capture is recorded for the workload."""
+    path = os.path.join(ROOT, TRAFFIC_CSV)
     if not os.path.exists(path):
-        return None
+        return None, None
     import csv
     with open(path) as f:
-        for row in csv.DictReader(f):
-            if row["workload"] == workload and row["kernel"] == kernel:
-                return float(row["dram_read_bytes"]) + float(row["dram_write_bytes"])
-    return None
+        rows = [r for r in csv.DictReader(l for l in f if not l.startswith("#"))]
+    for row in rows:
+        if row["workload"] == workload and row["kernel"] == kernel:
+            return (float(row["dram_read_bytes"]) + float(row["dram_write_bytes"]),
+                    f"recorded: {TRAFFIC_CSV} (ncu --set full of commit {row.get('commit', '?')}), not measured in this run")
+    return None, None
 
 
 class ClockSampler:
@@ -148,6 +155,51 @@ def reduce_over_ranks(ms_total, e2e_ms, state_ok, dist, device):
 def whole_job_grind(ms_step, cells_per_rank, world, neq):
     """ns per (cell x equation x RHS evaluation) of the whole job: every rank advances its own replica."""
     return ms_step * 1e6 / (cells_per_rank * world * neq * RHS_PER_STEP)
+
+
+def time_workload(B, torch, prob, q, local, steps, warmup, segment=0):
+    """K device-timed steps (CFL + RK3) of one workload with inputs resident in HBM; kernel times from the library's event
+    brackets.  Returns (ms per step, per-kernel profile, launches, state finite, ctx-free)."""
+    ctx = B.init_from_problem(prob, device=local, march_segment=segment)
+    try:
+        stream = torch.cuda.current_stream().cuda_stream
+        qd = torch.from_numpy(q).cuda()
+        for _ in range(max(3, warmup)):
+            B.mfc_rk3_step(ctx, qd.data_ptr(), B.mfc_cfl_dt(ctx, qd.data_ptr(), stream), stream)
+        torch.cuda.synchronize()
+        for kid in range(B.MFC_K_COUNT):
+            B.mfc_profile_get(ctx, kid, reset=True)
+        B.mfc_profile_enable(ctx, True)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(steps):
+            B.mfc_rk3_step(ctx, qd.data_ptr(), B.mfc_cfl_dt(ctx, qd.data_ptr(), stream), stream)
+        e1.record()
+        torch.cuda.synchronize()
+        prof = {}
+        for kid in range(B.MFC_K_COUNT):
+            n, ms = B.mfc_profile_get(ctx, kid, reset=True)
+            prof[B.KERNEL_NAMES[kid]] = {"launches": n, "ms_total": ms, "ms_avg": (ms / n if n else 0.0)}
+        B.mfc_profile_enable(ctx, False)
+        return e0.elapsed_time(e1) / steps, prof, bool(torch.isfinite(qd).all().item())
+    finally:
+        B.mfc_destroy(ctx)
+
+
+def extra_config_line(B, torch, name, prob, q, local, steps, fp64_tf, hbm_peak):
+    """One entry of `extra_configs`: the same step, event-timed, on a non-headline workload, with its roofline fractions."""
+    ms_step, prof, ok = time_workload(B, torch, prob, q, local, steps, 3)
+    flops_cell, bytes_cell = rhs_algorithmic(prob)
+    t_avg = prof["rhs_fused"]["ms_avg"] * 1e-3
+    return {"workload": f"{prob.name} {prob.n[0]}x{prob.n[1]}x{prob.n[2]} nf={prob.nf} neq={prob.neq} ({name})", "steps": steps,
+            "ms_per_step": ms_step, "value": ms_step * 1e6 / (prob.cells * prob.neq * RHS_PER_STEP), "unit": UNIT,
+            "cells_steps_per_s": prob.cells / (ms_step * 1e-3),
+            "kernels_ms_avg": {k: v["ms_avg"] for k, v in prof.items() if v["launches"]},
+            "roofline": {"kernel": "rhs_fused", "bound": "alu", "achieved": flops_cell * prob.cells / t_avg / 1e12, "peak": fp64_tf,
+                         "unit": "TFLOP/s", "frac": flops_cell * prob.cells / t_avg / 1e12 / fp64_tf,
+                         "hbm_frac": bytes_cell * prob.cells / t_avg / 1e9 / hbm_peak,
+                         "algorithmic_flops_per_cell": flops_cell, "algorithmic_bytes_per_cell": bytes_cell},
+            "state_finite": ok}
 
 
 def run_ours(args):
@@ -252,7 +304,8 @@ def run_ours(args):
         ach_tf = flops_cell * prob.cells / t_avg / 1e12
         t_hbm = bytes_cell * prob.cells / (hbm_peak * 1e9)
         t_alu = flops_cell * prob.cells / (fp64_tf * 1e12)
-        traffic = ncu_traffic(args.workload if not args.n else "", dom)
+        plain = not (args.n or args.kapila or args.stretched or args.segment)
+        traffic, traffic_src = ncu_traffic(args.workload if plain else "", dom)
         if t_hbm >= t_alu:
             roof = {"kernel": dom, "bound": "hbm", "achieved": ach_gbs, "peak": hbm_peak, "unit": "GB/s",
                     "frac": ach_gbs / hbm_peak, "traffic": traffic, "peak_source": f"MEASURED_PEAKS.json ({hbm_src})"}
@@ -263,7 +316,8 @@ def run_ours(args):
         roof.update({"algorithmic_flops_per_cell": flops_cell, "algorithmic_bytes_per_cell": bytes_cell,
                      "avg_launch_ms": prof[dom]["ms_avg"], "hbm_frac": ach_gbs / hbm_peak, "fp64_frac": ach_tf / fp64_tf,
                      "hbm_peak_gbs": hbm_peak, "hbm_peak_source": f"MEASURED_PEAKS.json ({hbm_src})",
-                     "traffic_source": "profiles/r01_dram_traffic.csv (ncu --set full)" if traffic else None,
+                     "traffic_source": traffic_src,
+                     "fp64_pipe_busy_recorded": "profiles/r02_ncu_full.md (sm__inst_executed_pipe_fp64, executed-flop fraction)",
                      "fp64_peak_measured_tflops": fp64_tf, "fp64_peak_nominal_tflops": FP64_NOMINAL_TFLOPS,
                      "kernel_ms_sum_over_step_ms": sum(v["ms_total"] for v in prof.values()) / ms_total})
         out = {
@@ -285,8 +339,23 @@ def run_ours(args):
         }
         if world == 1 and not args.no_cpu:
             out["cpu_baseline"] = cpu_baseline(args)
-        print(json.dumps(out))
     B.mfc_destroy(ctx)
+    del qd
+    torch.cuda.empty_cache()
+    if rank == 0:
+        if world == 1 and not args.no_extra and plain:
+            # non-headline workloads, event-timed the same way: the paper's ~2 M cells per device
+            # regime (cfg2), the three-fluid 384^3 case (cfg4) and the headline data on the Eq. 15 stretched grid
+            from paper_2305_09163_b200 import workloads as wl
+            extra = []
+            for name, make in (("BASELINE.json configs[2]", lambda: wl.cfg2()), ("BASELINE.json configs[4]", lambda: wl.cfg4()),
+                               ("configs[3] on the Eq. 15 stretched grid", lambda: (lambda pq: (wl.with_stretched_grid(pq[0]), pq[1]))(wl.cfg3()))):
+                p2, q2 = make()
+                extra.append(extra_config_line(B, torch, name, p2, q2, local, 5, fp64_tf, hbm_peak))
+                del q2
+                torch.cuda.empty_cache()
+            out["extra_configs"] = extra
+        print(json.dumps(out))
     if dist:
         dist.barrier()
         dist.destroy_process_group()
@@ -309,12 +378,36 @@ def oracle_step_time(args, n_sample: int, steps: int, warmup: int):
     return prob, times, oracle.threads()
 
 
+def cpu_model() -> str:
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
 def cpu_baseline(args):
+    """The oracle as it stands on the box's host cores: all cores (OpenMP on the outer loops) and ONE thread
+    (BASELINE.md section 3), on bounded samples of the headline workload; grind time is size-normalised."""
+    import oracle
     n_sample = args.cpu_n
     prob, times, cores = oracle_step_time(args, n_sample, 2, 0)
     sec = sum(times) / len(times)
+    oracle.set_threads(1)
+    try:
+        n1 = max(32, n_sample // 2)
+        prob1, times1, _ = oracle_step_time(args, n1, 1, 0)
+    finally:
+        oracle.set_threads(cores)
+    sec1 = times1[0]
     return {"value": sec * 1e9 / (prob.cells * prob.neq * RHS_PER_STEP), "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": f"{prob.name} shrunk to {n_sample}^3 cells, 2 steps of (CFL + RK3) with the OpenMP oracle, {sec:.2f} s/step"}
+            "sample": f"{prob.name} shrunk to {n_sample}^3 cells, 2 steps of (CFL + RK3) with the OpenMP oracle, {sec:.2f} s/step",
+            "cpu_model": cpu_model(),
+            "one_thread": {"value": sec1 * 1e9 / (prob1.cells * prob1.neq * RHS_PER_STEP), "unit": UNIT, "cores": 1,
+                           "sample": f"{prob1.name} shrunk to {n1}^3 cells, 1 step of (CFL + RK3), {sec1:.2f} s/step"}}
 
 
 def run_reference(args):
@@ -350,6 +443,7 @@ def main():
     ap.add_argument("--cpu-n", type=int, default=128, help="cells per dimension of the cpu_baseline sample")
     ap.add_argument("--ref-n", type=int, default=96, help="cells per dimension of the --impl reference sample")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-extra", action="store_true", help="skip the extra_configs leg (cfg2, cfg4, stretched cfg3)")
     ap.add_argument("--kapila", action="store_true", help="switch the K div(u) source of PAPER.md Eq. 2 on (not the headline config)")
     ap.add_argument("--stretched", action="store_true", help="same per-cell data on the Eq. 15 stretched grid (non-uniform spacing; not the headline config)")
     args = ap.parse_args()

@@ -29,11 +29,11 @@ def test_algorithmic_work_per_cell_matches_the_survey_counts():
 def test_committed_dram_traffic_is_at_least_the_compulsory_bytes():
     prob, _ = wl.cfg3(n=8)
     _, nbytes = bench.rhs_algorithmic(prob)
-    t = bench.ncu_traffic("cfg3", "rhs_fused")
-    assert t is not None
+    t, src = bench.ncu_traffic("cfg3", "rhs_fused")
+    assert t is not None and "recorded" in src and "commit" in src     # provenance: which commit the capture belongs to
     cells = 256 ** 3
     assert 1.0 <= t / (nbytes * cells) < 1.3          # re-reads stay small: each cell is read once (plus halos)
-    assert bench.ncu_traffic("cfg3", "no_such_kernel") is None and bench.ncu_traffic("", "rhs_fused") is None
+    assert bench.ncu_traffic("cfg3", "no_such_kernel") == (None, None) and bench.ncu_traffic("", "rhs_fused") == (None, None)
 
 
 def test_metric_and_unit_are_the_baseline_ones():
