@@ -57,7 +57,8 @@ typedef enum {
  * Non-uniform spacing ("structured mesh with non-uniform spacing"; Listing 1's per-index coefficient tables;
  * Eq. 15 stretching): edges_host[d] != NULL gives the n[d] + 1 strictly increasing cell edges of dimension d (host
  * pointer, copied by mfc_init; lo[d], hi[d] are then ignored); dimensions may be mixed.  A ghost cell has the width of the
- * cell its value is copied from (periodic: widths wrap; extrapolation: the boundary cell's width).  WENO5 only
+ * cell its value is copied from (periodic: widths wrap; extrapolation: the boundary cell's width); MFC_BC_HALO sides are
+ * not supported in a non-uniform dimension (MFC_EUNSUPPORTED: the ghost widths would be the neighbour's).  WENO5 only
  * (weno_order 5); the ideal weights of every cell must be positive (true for smooth stretching), else MFC_EUNSUPPORTED. */
 typedef struct {
     int ndim;        /* 1, 2 or 3 */
@@ -71,7 +72,13 @@ typedef struct {
     double gamma, pi_inf;
 } mfc_fluid;
 
-typedef enum { MFC_BC_PERIODIC = 0, MFC_BC_EXTRAP = 1 } mfc_bc_kind;
+typedef enum {
+    MFC_BC_PERIODIC = 0,
+    MFC_BC_EXTRAP = 1,
+    MFC_BC_HALO = 2 /* the ghost cells of this side belong to the caller: they hold a neighbouring block's cells (domain
+                       decomposition) or any fill of the caller's own; the library reads them, never
+                       writes them */
+} mfc_bc_kind;
 
 /* ghost-cell fills; periodic must be set on both sides of a dimension or on neither */
 typedef struct {
@@ -119,6 +126,14 @@ int mfc_rhs(mfc_ctx *ctx, double *q_dev, double *rhs_dev, void *stream);
  *   q1 = q + dt L(q);  q2 = 3/4 q + 1/4 (q1 + dt L(q1));  q <- 1/3 q + 2/3 (q2 + dt L(q2)).
  * On return the ghost cells of q_dev hold the boundary fill of the state the step STARTED from. */
 int mfc_rk3_step(mfc_ctx *ctx, double *q_dev, double dt, void *stream);
+
+/* The three stages of mfc_rk3_step one at a time (stage = 0, 1, 2, in this order), for callers that fill ghost cells
+ * between the stages (MFC_BC_HALO: halo exchange with neighbouring blocks):
+ *   stage 0 evaluates L on q_dev, stage 1 on the library's array q1, stage 2 on q2 (mfc_stage_array), and stage 2
+ *   writes the result into q_dev.  The array a stage evaluates L on must have its HALO ghost cells filled first. */
+int mfc_rk3_stage(mfc_ctx *ctx, int stage, double *q_dev, double dt, void *stream);
+/* Device pointer of the library's stage array k = 1, 2 (q1, q2; `elems` doubles, the layout of q). */
+int mfc_stage_array(mfc_ctx *ctx, int k, double **array_dev);
 
 /* CFL-restricted time step: dt = cfl * min over interior cells and directions of
  * dx_d / (|u_d| + c), c the frozen mixture sound speed (dx_d the cell's own width).  Synchronises `stream`; writes one

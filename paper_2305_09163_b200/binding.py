@@ -15,14 +15,15 @@ LIB_PATH = _HERE / "libmfc_b200.so"
 
 MFC_NG = 3
 MFC_OK, MFC_EINVAL, MFC_EUNSUPPORTED, MFC_ECUDA, MFC_ENOMEM, MFC_ENONFINITE = 0, -1, -2, -3, -4, -5
-MFC_BC_PERIODIC, MFC_BC_EXTRAP = 0, 1
+MFC_BC_PERIODIC, MFC_BC_EXTRAP, MFC_BC_HALO = 0, 1, 2
 MFC_K_RHS, MFC_K_CFL, MFC_K_PRIM, MFC_K_GHOST, MFC_K_COUNT = 0, 1, 2, 3, 4
 KERNEL_NAMES = {MFC_K_RHS: "rhs_fused", MFC_K_CFL: "cfl", MFC_K_PRIM: "prim", MFC_K_GHOST: "ghost_fill"}
 MFC_STAGING_AUTO, MFC_STAGING_TMA, MFC_STAGING_CPASYNC = 0, 1, 2
 
 # every symbol include/mfc.h declares
 EXPORTS = [
-    "mfc_init", "mfc_destroy", "mfc_layout", "mfc_rhs", "mfc_rk3_step", "mfc_cfl_dt", "mfc_advance_host",
+    "mfc_init", "mfc_destroy", "mfc_layout", "mfc_rhs", "mfc_rk3_step", "mfc_rk3_stage", "mfc_stage_array", "mfc_cfl_dt",
+    "mfc_advance_host",
     "mfc_cons_to_prim", "mfc_line_fluxes", "mfc_profile_enable", "mfc_profile_get", "mfc_launch_count",
     "mfc_probe_dfma", "mfc_strerror", "mfc_version", "mfc_cuda_error",
 ]
@@ -80,6 +81,8 @@ def lib():
     L.mfc_rhs.argtypes = [vp, vp, vp, vp]; L.mfc_rhs.restype = C.c_int
     L.mfc_rk3_step.argtypes = [vp, vp, C.c_double, vp]; L.mfc_rk3_step.restype = C.c_int
     L.mfc_cfl_dt.argtypes = [vp, vp, dp, vp]; L.mfc_cfl_dt.restype = C.c_int
+    L.mfc_rk3_stage.argtypes = [vp, C.c_int, vp, C.c_double, vp]; L.mfc_rk3_stage.restype = C.c_int
+    L.mfc_stage_array.argtypes = [vp, C.c_int, C.POINTER(vp)]; L.mfc_stage_array.restype = C.c_int
     L.mfc_advance_host.argtypes = [vp, vp, C.c_int, C.c_double, dp, vp]; L.mfc_advance_host.restype = C.c_int
     L.mfc_cons_to_prim.argtypes = [vp, vp, vp, vp]; L.mfc_cons_to_prim.restype = C.c_int
     L.mfc_line_fluxes.argtypes = [vp, C.c_int, C.c_int, vp, vp, vp, vp, vp, vp]; L.mfc_line_fluxes.restype = C.c_int
@@ -168,6 +171,17 @@ def mfc_rhs(ctx, q_dev: int, rhs_dev: int, stream: int = 0) -> None:
 
 def mfc_rk3_step(ctx, q_dev: int, dt: float, stream: int = 0) -> None:
     _check_ctx(lib().mfc_rk3_step(ctx, q_dev, float(dt), stream), "mfc_rk3_step", ctx)
+
+
+def mfc_rk3_stage(ctx, stage: int, q_dev: int, dt: float, stream: int = 0) -> None:
+    _check_ctx(lib().mfc_rk3_stage(ctx, int(stage), q_dev, float(dt), stream), "mfc_rk3_stage", ctx)
+
+
+def mfc_stage_array(ctx, k: int) -> int:
+    """-> device address of the library's stage array q1 (k = 1) or q2 (k = 2)"""
+    p = C.c_void_p()
+    _check(lib().mfc_stage_array(ctx, int(k), C.byref(p)), "mfc_stage_array")
+    return int(p.value)
 
 
 def mfc_cfl_dt(ctx, q_dev: int, stream: int = 0) -> float:

@@ -222,12 +222,14 @@ int cuda_to_status(cudaError_t e, mfc_ctx *c = nullptr)
 // out = base + coef L(q_in), base described by `o` (SweepOut, mfc_launch.h).
 int eval_L(mfc_ctx *c, double *q_in, const SweepOut &o, cudaStream_t s)
 {
-    cudaError_t err;
-    {
+    cudaError_t err = cudaSuccess;
+    bool all_halo = true;
+    for (int d = 0; d < c->ndim; ++d) all_halo = all_halo && c->g.bc_lo[d] == MFC_BC_HALO && c->g.bc_hi[d] == MFC_BC_HALO;
+    if (!all_halo) {
         Timed t(c, MFC_K_GHOST, s);
         err = launch_ghost_fill(c->g, c->neq, q_in, s);
+        if (err != cudaSuccess) return cuda_to_status(err, c);
     }
-    if (err != cudaSuccess) return cuda_to_status(err, c);
     {
         Timed t(c, MFC_K_RHS, s);
         err = launch_rhs(c->ndim, c->nf, c->order, c->g, c->e, q_in, o, c->segment, c->staging, s);
@@ -237,20 +239,30 @@ int eval_L(mfc_ctx *c, double *q_in, const SweepOut &o, cudaStream_t s)
 
 // 3-stage TVD Runge-Kutta.  Every stage is out = ca qn + cb (qs + dt L(qs)).  A stage reads its
 // neighbours' cells of qs, so it never writes the array it evaluates L on: q -> q1 -> q2 -> q.
-int rk3(mfc_ctx *c, double *q, double dt, cudaStream_t s)
+int rk3_stage(mfc_ctx *c, int stage, double *q, double dt, cudaStream_t s)
 {
     SweepOut f{};
-    // q1 = q + dt L(q)
-    f.out = c->q1; f.qs = q; f.qn = q; f.ca = 0.0; f.cb = 1.0; f.coef = dt; f.nbase = 1;
-    int st = eval_L(c, q, f, s);
-    if (st) return st;
-    // q2 = 3/4 q + 1/4 (q1 + dt L(q1))
-    f.out = c->q2; f.qs = c->q1; f.qn = q; f.ca = 0.75; f.cb = 0.25; f.coef = 0.25 * dt; f.nbase = 2;
-    st = eval_L(c, c->q1, f, s);
-    if (st) return st;
-    // q <- 1/3 q + 2/3 (q2 + dt L(q2))
-    f.out = q; f.qs = c->q2; f.qn = q; f.ca = 1.0 / 3.0; f.cb = 2.0 / 3.0; f.coef = (2.0 / 3.0) * dt; f.nbase = 2;
-    return eval_L(c, c->q2, f, s);
+    switch (stage) {
+        case 0:   // q1 = q + dt L(q)
+            f.out = c->q1; f.qs = q; f.qn = q; f.ca = 0.0; f.cb = 1.0; f.coef = dt; f.nbase = 1;
+            return eval_L(c, q, f, s);
+        case 1:   // q2 = 3/4 q + 1/4 (q1 + dt L(q1))
+            f.out = c->q2; f.qs = c->q1; f.qn = q; f.ca = 0.75; f.cb = 0.25; f.coef = 0.25 * dt; f.nbase = 2;
+            return eval_L(c, c->q1, f, s);
+        case 2:   // q <- 1/3 q + 2/3 (q2 + dt L(q2))
+            f.out = q; f.qs = c->q2; f.qn = q; f.ca = 1.0 / 3.0; f.cb = 2.0 / 3.0; f.coef = (2.0 / 3.0) * dt; f.nbase = 2;
+            return eval_L(c, c->q2, f, s);
+    }
+    return MFC_EINVAL;
+}
+
+int rk3(mfc_ctx *c, double *q, double dt, cudaStream_t s)
+{
+    for (int stage = 0; stage < 3; ++stage) {
+        const int st = rk3_stage(c, stage, q, dt, s);
+        if (st) return st;
+    }
+    return MFC_OK;
 }
 
 int cfl_dt(mfc_ctx *c, const double *q, double *dt_host, cudaStream_t s)
@@ -420,12 +432,14 @@ int mfc_init(mfc_ctx **out, const mfc_grid *grid, int n_fluids, const mfc_fluid 
     for (int d = 0; d < grid->ndim; ++d) {
         if (grid->n[d] < MFC_NG) return MFC_EINVAL;
         if (grid->edges_host[d]) {
+            // the widths of HALO ghost cells are the neighbour's: not expressible through edges_host yet
+            if (bc->lo[d] == MFC_BC_HALO || bc->hi[d] == MFC_BC_HALO) return MFC_EUNSUPPORTED;
             nonuniform = true;
             for (int i = 0; i < grid->n[d]; ++i)
                 if (!(grid->edges_host[d][i + 1] > grid->edges_host[d][i]) || !std::isfinite(grid->edges_host[d][i + 1] - grid->edges_host[d][i])) return MFC_EINVAL;
         } else if (!(grid->hi[d] > grid->lo[d])) return MFC_EINVAL;
-        if (bc->lo[d] != MFC_BC_PERIODIC && bc->lo[d] != MFC_BC_EXTRAP) return MFC_EINVAL;
-        if (bc->hi[d] != MFC_BC_PERIODIC && bc->hi[d] != MFC_BC_EXTRAP) return MFC_EINVAL;
+        if (bc->lo[d] < MFC_BC_PERIODIC || bc->lo[d] > MFC_BC_HALO) return MFC_EINVAL;
+        if (bc->hi[d] < MFC_BC_PERIODIC || bc->hi[d] > MFC_BC_HALO) return MFC_EINVAL;
         if ((bc->lo[d] == MFC_BC_PERIODIC) != (bc->hi[d] == MFC_BC_PERIODIC)) return MFC_EINVAL;
     }
     if (nonuniform && order != 5) return MFC_EUNSUPPORTED;
@@ -577,6 +591,20 @@ int mfc_rk3_step(mfc_ctx *c, double *q_dev, double dt, void *stream)
     if (!c || !q_dev) return MFC_EINVAL;
     DeviceGuard guard(c->device);
     return rk3(c, q_dev, dt, (cudaStream_t)stream);
+}
+
+int mfc_rk3_stage(mfc_ctx *c, int stage, double *q_dev, double dt, void *stream)
+{
+    if (!c || !q_dev || stage < 0 || stage > 2) return MFC_EINVAL;
+    DeviceGuard guard(c->device);
+    return rk3_stage(c, stage, q_dev, dt, (cudaStream_t)stream);
+}
+
+int mfc_stage_array(mfc_ctx *c, int k, double **array_dev)
+{
+    if (!c || !array_dev || (k != 1 && k != 2)) return MFC_EINVAL;
+    *array_dev = k == 1 ? c->q1 : c->q2;
+    return MFC_OK;
 }
 
 int mfc_cfl_dt(mfc_ctx *c, const double *q_dev, double *dt_host, void *stream)

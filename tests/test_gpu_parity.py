@@ -664,6 +664,52 @@ def test_step_runs_beside_a_tensor_core_kernel_on_another_stream():
 
 
 # ---------------------------------------------------------------------------------------------
+# block decomposition: one block that is its own neighbour == the single-block solver
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("ndim,n,periodic_dims", [(2, (70, 45), (0,)), (3, (40, 29, 33), (0, 1, 2)), (3, (41, 30, 33), (1,)), (3, (40, 29, 33), ())])
+def test_block_solver_with_halo_ghosts_reproduces_the_single_block_solver(ndim, n, periodic_dims):
+    """MFC_BC_HALO on every side + halo.fill_ghosts (local wrap / edge copies for a 1 x 1 x 1 decomposition) through
+    mfc_rhs and the per-stage mfc_rk3_stage gives the bits of the ordinary context: the kernels read the ghost cells the
+    caller filled, whatever the staging path (TMA at n[0] = 40, cp.async at 41)."""
+    import dataclasses
+    from paper_2305_09163_b200 import halo
+    prob, q = wl.random_state(ndim, n, 2, seed=90 + ndim, periodic=True)
+    bc = tuple(wl.BC_PERIODIC if d in periodic_dims else wl.BC_EXTRAP for d in range(3))
+    prob = dataclasses.replace(prob, bc_lo=bc, bc_hi=bc)
+    orc = oracle.Oracle(prob)
+    dts = [0.7 * orc.cfl_dt(q.copy(), prob.cfl)] * 3
+    it = prob.interior()
+    with Gpu(prob) as g:
+        torch = g.torch
+        L_ref = g.rhs(q)[it]
+        q_ref = g.rk3(q, dts)[it]
+        dt_ref = g.cfl_dt(q)
+        dec = halo.Decomposition((1, 1, 1), prob.bc_lo, prob.bc_hi)
+        blk = halo.BlockSolver(prob, dec, 0)
+        try:
+            qd = g.to_dev(q)
+            out = torch.zeros_like(qd)
+            blk.rhs(qd, out)
+            assert blk.cfl_dt(qd) == dt_ref
+            for dt in dts:
+                blk.rk3_step(qd, dt)
+            torch.cuda.synchronize()
+            assert np.array_equal(out.cpu().numpy()[it], L_ref)
+            assert np.array_equal(qd.cpu().numpy()[it], q_ref)
+        finally:
+            blk.close()
+
+
+def test_halo_sides_are_refused_in_a_non_uniform_dimension():
+    import dataclasses
+    prob, q = wl.random_state(2, (20, 12), 2, seed=1)
+    ps = dataclasses.replace(wl.with_stretched_grid(prob), bc_lo=(B.MFC_BC_HALO,) * 3, bc_hi=(B.MFC_BC_HALO,) * 3)
+    with pytest.raises(B.MfcError) as ei:
+        Gpu(ps)
+    assert ei.value.code == B.MFC_EUNSUPPORTED
+
+
+# ---------------------------------------------------------------------------------------------
 # host-buffer entry point and measurement hooks
 # ---------------------------------------------------------------------------------------------
 def test_advance_host_equals_device_path():
