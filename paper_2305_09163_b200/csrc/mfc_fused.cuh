@@ -38,7 +38,7 @@
 namespace mfc {
 
 #ifndef MFC_XPRE
-#define MFC_XPRE 4   // variables whose x reconstruction runs before the first barrier of the in-plane part (measured: 4 best)
+#define MFC_XPRE 2   // variables whose x reconstruction runs before the first barrier of the in-plane part (measured on the TMA kernel at cfg3: 0: 2.585, 1: 2.563, 2: 2.548, 3: 2.573, 4: 2.572, 6: 2.603, 7: 2.619 ms)
 #endif
 constexpr int FTX = 32;             // tile width in x = warp width
 constexpr int FPX = FTX + 2 * NG;   // staged row length
