@@ -64,11 +64,13 @@ struct FusedCfg {
     // rim in y, per column: vL of row -1, vR of row TY; the rim flux overwrites them likewise
     static constexpr int nHy = D >= 2 ? 2 * NEQ * FTX : 0;
     static constexpr int nX8 = D >= 2 ? NT : 0;                     // face velocity row of the y exchange
-    // 1D / 2D: the y exchange has its own buffer.  3D: it lives in the ring slot of the plane staged in P;
-    // ring (4 slots) + parked left state + staging of raw q: own column of the next plane, q_s of the cell being
-    // written, halo cells of the next two staged planes (double buffer)
+    // y exchange: right states X and fluxes X2, [NEQ][NT] each.  X is written before barrier S1 and read between S1 and
+    // S2; X2 (and X8) are written before S2 and read after it; both are free again after the barrier that ends the
+    // iteration.  3D (cp.async kernel) adds the staging of raw q: own column of the next plane (SQ), q_s of the cell being
+    // written (SS), halo cells of the next two staged planes (SH, double buffer).  The z window (ring of four primitive
+    // planes, parked left state, previous flux) lives in tensor memory, not here.
     static constexpr int nX = D == 2 ? 2 * NEQ * NT : 0;
-    static constexpr int nR = D == 3 ? 2 * NEQ * NT + 2 : 0;        // y exchange buffers + the TMEM base word (ring, park: in TMEM)
+    static constexpr int nR = D == 3 ? 2 * NEQ * NT + 2 : 0;        // X, X2 + the TMEM base word
     static constexpr int nS = D == 3 ? NEQ * (2 * NT + 2 * NH) : 0;
     static constexpr int doubles = nP + nHx + nHy + nX8 + nX + nR + nS;
     static constexpr int bytes = doubles * (int)sizeof(double);
@@ -411,7 +413,6 @@ __global__ void __launch_bounds__(FTX *TY, 1)
     using C = FusedCfg<D, NF, TY>;
     using I = Idx<D, NF>;
     constexpr int NEQ = C::NEQ, NT = C::NT, PPL = C::PPL, NH = C::NH, NHT = C::NHT;
-    constexpr int NA1 = I::NA > 0 ? I::NA : 1;
     extern __shared__ double sm[];
     double *const P = sm;
     double *const rim = P + C::nP;
@@ -534,7 +535,7 @@ __global__ void __launch_bounds__(FTX *TY, 1)
     //   bottom   z part from wn = SQ; plane m -> ring; out(ip) written  ||  glue: P restaged with plane ip + 1 (own
     //            cell from the ring, halo cells from SH); issue, as three commit groups in this order, {q_s of cell
     //            ip + 1}, {raw column m + 1}, {raw halo of plane m = ip + 3}   (order of the two halves per warp group)
-    //   barrier  (P staged; the exchange buffer, which is the ring slot plane m + 1 goes to, is free)
+    //   barrier  (P is staged; X, X2 and the rim buffers are free again)
     // The conversions need everything but the youngest group (the halo issued one iteration ago is used two
     // iterations after its issue), so the only wait is "all but the youngest", half an iteration after the issue
     // of q_s (L2-resident: it was this block's column three planes ago) and of the column.
@@ -599,7 +600,7 @@ __global__ void __launch_bounds__(FTX *TY, 1)
             }
         }
         // plane m of the own column (primitives since the conversion above) and plane m - 3 = ip: the latter sits in P
-        // when it has just been differenced in plane (its ring slot was the exchange buffer)
+        // when it has just been differenced in plane, else in its ring slot
         double wn[TV], vb[TV];
 #pragma unroll
         for (int k = NEQ; k < TV; ++k) { wn[k] = 0.0; vb[k] = 0.0; }
@@ -698,7 +699,7 @@ __global__ void __launch_bounds__(FTX *TY, 1)
             zpart();
             glue();
         }
-        __syncthreads();                                            // P is staged, the exchange buffer is free
+        __syncthreads();                                            // P is staged; X, X2 and the rim buffers are free
     }
     if (j == 0) tmem_dealloc512(tmem_base);
 }
