@@ -18,7 +18,7 @@ MFC_OK, MFC_EINVAL, MFC_EUNSUPPORTED, MFC_ECUDA, MFC_ENOMEM, MFC_ENONFINITE = 0,
 MFC_BC_PERIODIC, MFC_BC_EXTRAP, MFC_BC_HALO = 0, 1, 2
 MFC_K_RHS, MFC_K_CFL, MFC_K_PRIM, MFC_K_GHOST, MFC_K_COUNT = 0, 1, 2, 3, 4
 KERNEL_NAMES = {MFC_K_RHS: "rhs_fused", MFC_K_CFL: "cfl", MFC_K_PRIM: "prim", MFC_K_GHOST: "ghost_fill"}
-MFC_STAGING_AUTO, MFC_STAGING_TMA, MFC_STAGING_CPASYNC = 0, 1, 2
+MFC_STAGING_AUTO, MFC_STAGING_TMA, MFC_STAGING_CPASYNC, MFC_STAGING_ROLES = 0, 1, 2, 3
 
 # every symbol include/mfc.h declares
 EXPORTS = [

@@ -19,7 +19,7 @@ CSRC = HERE / "csrc"
 OBJ = HERE / "build"
 LIB = HERE / "libmfc_b200.so"
 SOURCES = ["mfc_api.cu", "mfc_inst_d1.cu", "mfc_inst_d2.cu", "mfc_inst_d3.cu"]
-HEADERS = [CSRC / "mfc_math.cuh", CSRC / "mfc_kernels.cuh", CSRC / "mfc_fused.cuh", CSRC / "mfc_fused_tma.cuh", CSRC / "mfc_launch.h", CSRC / "mfc_inst.cuh", HERE.parent / "include" / "mfc.h"]
+HEADERS = [CSRC / "mfc_math.cuh", CSRC / "mfc_kernels.cuh", CSRC / "mfc_fused.cuh", CSRC / "mfc_fused_tma.cuh", CSRC / "mfc_fused_roles.cuh", CSRC / "mfc_launch.h", CSRC / "mfc_inst.cuh", HERE.parent / "include" / "mfc.h"]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "--fmad=true"]
 # extra flags for experiments (e.g. MFC_NVCC_EXTRA="-DMFC_XPRE=2"); the committed numbers are measured without any

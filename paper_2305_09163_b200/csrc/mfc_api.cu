@@ -427,7 +427,7 @@ int mfc_init(mfc_ctx **out, const mfc_grid *grid, int n_fluids, const mfc_fluid 
     if (opts && opts->kapila && n_fluids != 2) return MFC_EUNSUPPORTED;
     const int order = (opts && opts->weno_order != 0) ? opts->weno_order : 5;
     if (order != 1 && order != 3 && order != 5) return MFC_EINVAL;
-    if (opts && (opts->staging < 0 || opts->staging > 2)) return MFC_EINVAL;
+    if (opts && (opts->staging < 0 || opts->staging > 3)) return MFC_EINVAL;
     bool nonuniform = false;
     for (int d = 0; d < grid->ndim; ++d) {
         if (grid->n[d] < MFC_NG) return MFC_EINVAL;

@@ -3,6 +3,7 @@
 #include "mfc_kernels.cuh"
 #include "mfc_fused.cuh"
 #include "mfc_fused_tma.cuh"
+#include "mfc_fused_roles.cuh"
 
 #ifndef MFC_D
 #error "define MFC_D (1, 2 or 3) before including mfc_inst.cuh"
@@ -122,6 +123,18 @@ static cudaError_t launch_fused_nu(const typename GeoOf<NU>::type &g, const Eos 
         const bool tma_ok = path != MFC_PATH_LDGSTS && (g.p[0] & 1) == 0 && (reinterpret_cast<unsigned long long>(q) & 15) == 0 &&
                             (o.nbase == 0 || o.qs == q);
         CUtensorMap tm_plane, tm_col;
+        // warp-specialised kernel (mfc_fused_roles.cuh): uniform grid, two fluids, the TMA layout conditions
+        if constexpr (!NU && NF == 2 && TY == 12) {
+            if (path == MFC_PATH_ROLES) {
+                using R = RolesCfg<NF, TY>;
+                static_assert(R::bytes <= 227 * 1024, "role-split tile does not fit shared memory");
+                if (!tma_ok || !encode_state_map(&tm_plane, g, C::NEQ, q, FPX, C::PY) || !encode_state_map(&tm_col, g, C::NEQ, q, R::CW, 1))
+                    return cudaErrorInvalidValue;
+                if ((st = MFC_OPTIN_SHARED((rhs_fused_roles_kernel<NF, TY, ORDER>), R::bytes)) != cudaSuccess) return st;
+                rhs_fused_roles_kernel<NF, TY, ORDER><<<blocks, R::THREADS, R::bytes, s>>>(tm_plane, tm_col, g, e, o, ntx, nty, seg);
+                return cudaSuccess;
+            }
+        } else if (path == MFC_PATH_ROLES) return cudaErrorInvalidValue;
         if (tma_ok && encode_state_map(&tm_plane, g, C::NEQ, q, FPX, C::PY) && encode_state_map(&tm_col, g, C::NEQ, q, T::CW, TY)) {
             if ((st = MFC_OPTIN_SHARED((rhs_fused_march_tma_kernel<NF, TY, ORDER, NU>), T::bytes)) != cudaSuccess) return st;
             rhs_fused_march_tma_kernel<NF, TY, ORDER, NU><<<blocks, C::NT, T::bytes, s>>>(tm_plane, tm_col, g, e, o, ntx, nty, seg);
