@@ -111,7 +111,16 @@ struct NuPlane {
 // `early` runs at the top of the first FP64-heavy block and `mid` at the top of the second: the caller's loads,
 // cp.async issues and the cons->prim chains of the NEXT plane go there, so that they overlap this plane's
 // arithmetic instead of forming latency-bound phases of their own.
-template <int D, int NF, int TY, int ORDER, bool NU = false, class Early = NoHook, class Mid = NoHook>
+// GT = 0: the two barriers inside are block barriers; GT > 0: barriers of the first GT threads only (bar.sync 1, GT), for
+// kernels whose remaining warps run another loop (mfc_fused_roles.cuh)
+template <int GT>
+__device__ __forceinline__ void inplane_sync()
+{
+    if constexpr (GT == 0) __syncthreads();
+    else asm volatile("bar.sync 1, %0;" ::"n"(GT) : "memory");
+}
+
+template <int D, int NF, int TY, int ORDER, bool NU = false, int GT = 0, class Early = NoHook, class Mid = NoHook>
 __device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, const Eos &eos, double cx, double cy,
                                            double (&acc)[2 * NF + D], Early early = Early(), Mid mid = Mid(),
                                            const NuPlane &nup = NuPlane{nullptr, nullptr, 0, 0})
@@ -198,7 +207,7 @@ __device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, cons
         const double *s5 = pc + e * PPL;
         reconstruct<ORDER, NU>(s5[0], s5[-1] - s5[-2], s5[0] - s5[-1], s5[1] - s5[0], s5[2] - s5[1], eos.weno_eps4, vL[e], vR[e], NuRef{nup.tx + i, nup.sx});
     }
-    __syncthreads();                                                // S1: rim states and y right states are visible
+    inplane_sync<GT>();                                             // S1: rim states and y right states are visible
 
     // ---- x: reconstruct, exchange by shuffles, solve face i + 1/2, difference ----
     mid();
@@ -261,7 +270,7 @@ __device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, cons
         for (int e = 0; e < NEQ; ++e) B.X2[e * NT + tid] = Fy[e];
         B.X8[tid] = ufy;
     }
-    __syncthreads();                                                // S2: fluxes (rim ones included) are visible
+    inplane_sync<GT>();                                             // S2: fluxes (rim ones included) are visible
     if (i == 0) {
         const double du = B.ExF[NEQ * TY + j] - FxH[NEQ * TY + j];
 #pragma unroll
