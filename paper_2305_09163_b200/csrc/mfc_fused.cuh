@@ -120,7 +120,9 @@ __device__ __forceinline__ void inplane_sync()
     else asm volatile("bar.sync 1, %0;" ::"n"(GT) : "memory");
 }
 
-template <int D, int NF, int TY, int ORDER, bool NU = false, int GT = 0, class Early = NoHook, class Mid = NoHook>
+// XP: variables whose x reconstruction runs before barrier S1; RIMBAL: the two warps that solve the rim faces between S1 and
+// S2 reconstruct one more variable before S1 than the others (their extra Riemann solve no longer delays S2 for everybody)
+template <int D, int NF, int TY, int ORDER, bool NU = false, int GT = 0, int XP = MFC_XPRE, bool RIMBAL = false, class Early = NoHook, class Mid = NoHook>
 __device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, const Eos &eos, double cx, double cy,
                                            double (&acc)[2 * NF + D], Early early = Early(), Mid mid = Mid(),
                                            const NuPlane &nup = NuPlane{nullptr, nullptr, 0, 0})
@@ -200,12 +202,18 @@ __device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, cons
     }
     // the x reconstruction needs nothing of the other warps: it runs BEFORE the barrier for the first XPRE variables,
     // so that the barrier's skew and the burst of stencil loads behind it are covered by arithmetic
-    constexpr int XPRE = NEQ < MFC_XPRE ? NEQ : MFC_XPRE;
+    constexpr int XPRE = NEQ < XP ? NEQ : XP;
+    const bool rim_early = RIMBAL && XPRE < NEQ && (j == RIMW || j == RIMX);
     double vL[NEQ], vR[NEQ];
 #pragma unroll
     for (int e = 0; e < XPRE; ++e) {
         const double *s5 = pc + e * PPL;
         reconstruct<ORDER, NU>(s5[0], s5[-1] - s5[-2], s5[0] - s5[-1], s5[1] - s5[0], s5[2] - s5[1], eos.weno_eps4, vL[e], vR[e], NuRef{nup.tx + i, nup.sx});
+    }
+    if (rim_early) {
+        const double *s5 = pc + XPRE * PPL;
+        reconstruct<ORDER, NU>(s5[0], s5[-1] - s5[-2], s5[0] - s5[-1], s5[1] - s5[0], s5[2] - s5[1], eos.weno_eps4, vL[XPRE < NEQ ? XPRE : 0], vR[XPRE < NEQ ? XPRE : 0],
+                               NuRef{nup.tx + i, nup.sx});
     }
     inplane_sync<GT>();                                             // S1: rim states and y right states are visible
 
@@ -215,6 +223,7 @@ __device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, cons
     {
 #pragma unroll
         for (int e = XPRE; e < NEQ; ++e) {
+            if (e == XPRE && rim_early) continue;
             const double *s5 = pc + e * PPL;
             reconstruct<ORDER, NU>(s5[0], s5[-1] - s5[-2], s5[0] - s5[-1], s5[1] - s5[0], s5[2] - s5[1], eos.weno_eps4, vL[e], vR[e], NuRef{nup.tx + i, nup.sx});
         }

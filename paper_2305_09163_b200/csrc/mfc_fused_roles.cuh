@@ -2,11 +2,12 @@
 // same decomposition as rhs_fused_march_tma_kernel (tile of 32 x TY cells in (x, y), march along z three planes ahead,
 // TMA-staged planes, z window in tensor memory), but the block has two kinds of warps, each with a loop of its own:
 //   in-plane warps (TY, one row each): the x and y differences of the staged plane (inplane_xy, mfc_fused.cuh, its two
-//       barriers now barriers of these warps only), the halo cons->prim of the next plane, and a4 + a5: Lx + Ly in
-//       registers + Lz from shared memory, the Runge-Kutta combine and the one store of the cell;
+//       barriers now barriers of these warps only) and a4 + a5: Lx + Ly in registers + Lz from shared memory, the
+//       Runge-Kutta combine and the one store of the cell;
 //   Z warps (TY / ZR, ZR rows each): raw row of plane m (TMA box, re-issued by the warp as soon as it has read it) ->
 //       primitives -> ring of four planes in tensor memory; cell m - 2 reconstructed, face solved against the parked left
-//       state, difference -> Lz (shared memory, two buffers); own cells of plane m - 2 written into the staged plane.
+//       state, difference -> Lz (shared memory, two buffers); own cells of plane m - 2 written into the staged plane,
+//       whose halo cells (landed raw) they convert in place.
 // The two kinds meet only through mbarriers (PRIM_P: own cells of a staged plane are primitives; FULL_LZ / EMPTY_LZ), so the
 // z part -- a latency-bound chain (tensor-memory loads, one Riemann solve) that ran at half the FP64 rate when all warps
 // of a scheduler were in it at once -- now overlaps the in-plane arithmetic of the other warps of its scheduler, and the
@@ -16,6 +17,13 @@
 #pragma once
 #include <cstdio>
 #include "mfc_fused_tma.cuh"
+
+#ifndef MFC_ROLES_XPRE
+#define MFC_ROLES_XPRE 4    // x reconstructions before barrier S1 (0 .. 7: 2.380 2.355 2.385 2.361 2.353 . . 2.414 ms at cfg3)
+#endif
+#ifndef MFC_ROLES_RIMBAL
+#define MFC_ROLES_RIMBAL false
+#endif
 
 namespace mfc {
 
@@ -78,7 +86,7 @@ template <int NF, int TY>
 struct RolesCfg {
     using C = FusedCfg<3, NF, TY>;
     static constexpr int NEQ = C::NEQ, NT = C::NT, PPL = C::PPL, NH = C::NH, NHT = C::NHT;
-    static constexpr int ZR = 3;                                         // rows per Z warp
+    static constexpr int ZR = TY / 4;                                         // rows per Z warp
     static constexpr int NZ = TY / ZR;                                   // Z warps
     static constexpr int WARPS = TY + NZ, THREADS = 32 * WARPS;
     static constexpr int CW = FTX + 2;                                   // own-row box: cells -1 .. FTX of one row, all variables
@@ -92,7 +100,8 @@ struct RolesCfg {
     static constexpr int oX2 = oX + NEQ * NT;                            //             fluxes [NEQ][NT]
     static constexpr int nL = NEQ * NT;
     static constexpr int oLz = r16(oX2 + NEQ * NT);                      // z flux differences [2][NEQ][NT]
-    static constexpr int oBar = oLz + 2 * nL;
+    static constexpr int NLZ = TY > 12 ? 1 : 2;
+    static constexpr int oBar = oLz + NLZ * nL;
     enum { FULL_P = 0, PRIM_P = 2, FULL_LZ = 4, EMPTY_LZ = 6, FULL_SQ = 8, NBAR = FULL_SQ + TY, TMEM_WORD = NBAR, NWORDS = NBAR + 1 };
     static constexpr int doubles = oBar + r16(NWORDS);
     static constexpr int bytes = doubles * (int)sizeof(double);
@@ -117,7 +126,7 @@ __global__ void __launch_bounds__(RolesCfg<NF, TY>::THREADS, 1)
     using R = RolesCfg<NF, TY>;
     using C = FusedCfg<D, NF, TY>;
     using I = Idx<D, NF>;
-    constexpr int NEQ = R::NEQ, NT = R::NT, PPL = R::PPL, NH = R::NH, NHT = R::NHT, CW = R::CW, TV = R::TV;
+    constexpr int NEQ = R::NEQ, NT = R::NT, PPL = R::PPL, NH = R::NH, CW = R::CW, TV = R::TV;
     extern __shared__ __align__(128) double sm[];
     double *const SQ = sm + R::oSQ;
     unsigned long long *const bars = reinterpret_cast<unsigned long long *>(sm + R::oBar);
@@ -151,6 +160,8 @@ __global__ void __launch_bounds__(RolesCfg<NF, TY>::THREADS, 1)
     const unsigned tmem_base = *tmem_word;
 
     auto par = [](int k) -> unsigned { return (unsigned)(k & 1); };    // phase parity of the k-th use of a barrier
+    auto lzb = [](int u) -> int { return R::NLZ == 2 ? (u & 1) : 0; };  // Lz buffer of plane u, and which use of it that is
+    auto lzk = [](int u) -> int { return R::NLZ == 2 ? (u >> 1) : u; };
     auto load_plane = [&](int v) {                                  // plane k0 + v with its halo -> P[v & 1] (one thread)
         mbar_expect_tx(bars + R::FULL_P + (v & 1), R::plane_bytes);
         tma_load_4d(sm + (v & 1) * R::nPb, &tm_plane, bars + R::FULL_P + (v & 1), x0, y0, k0 + v + NG, 0);
@@ -166,40 +177,10 @@ __global__ void __launch_bounds__(RolesCfg<NF, TY>::THREADS, 1)
         const int i = lane, j = warp;
         const bool active = x0 + i < g.n[0] && y0 + j < g.n[1];
         const long long col = (long long)(y0 + j + NG) * g.sy + (x0 + i + NG);
-        // halo cells of this thread: position in the staged plane (row-major numbering that skips the interior block)
-        int hpos[NHT];
-#pragma unroll
-        for (int t = 0; t < NHT; ++t) {
-            const int h = tid + t * NT;
-            constexpr int TOP = NG * FPX;
-            int c = 0;
-            if (h < TOP) c = h;
-            else if (h < TOP + 2 * NG * TY) {
-                const int r = (h - TOP) / (2 * NG), k = (h - TOP) - r * 2 * NG;
-                c = (NG + r) * FPX + (k < NG ? k : FTX + k);
-            } else if (h < NH) c = (NG + TY) * FPX + (h - TOP - 2 * NG * TY);
-            hpos[t] = c;
-        }
-        auto convert_halo = [&](double *Pb) {                       // cons->prim in place, this thread's halo cells of a landed plane
-#pragma unroll
-            for (int t = 0; t < NHT; ++t) {
-                if (tid + t * NT < NH) {
-                    double qc[NEQ], wc[NEQ];
-#pragma unroll
-                    for (int e = 0; e < NEQ; ++e) qc[e] = Pb[e * PPL + hpos[t]];
-                    cons_to_prim_cell<D, NF>(qc, eos, wc);
-#pragma unroll
-                    for (int e = 0; e < NEQ; ++e) Pb[e * PPL + hpos[t]] = wc[e];
-                }
-            }
-        };
         if (tid == 0) {                                             // both staged-plane buffers are free at the start
             load_plane(0);
             if (U > 1) load_plane(1);
         }
-        RWAIT(bars + R::FULL_P, 0);
-        convert_halo(sm);
-        inplane_sync<NT>();
         const InplaneBufs<D, NF, TY> B0(sm, sm + R::oRim, sm + R::oX, sm + R::oX2, sm + R::oX8);
         const InplaneBufs<D, NF, TY> B1(sm + R::nPb, sm + R::oRim, sm + R::oX, sm + R::oX2, sm + R::oX8);
 #pragma unroll 1
@@ -209,7 +190,7 @@ __global__ void __launch_bounds__(RolesCfg<NF, TY>::THREADS, 1)
             double coef = o.coef;
             asm volatile("" : "+d"(coef));
             const double cx = coef * g.inv_dx[0], cy = coef * g.inv_dx[1];
-            RWAIT(bars + R::PRIM_P + b, par(u >> 1));                  // the Z warps have written the own cells of plane u
+            RWAIT(bars + R::PRIM_P + b, par(u >> 1));                  // the Z warps have made plane u primitives (own cells and halo)
             double acc[NEQ];
 #pragma unroll
             for (int e = 0; e < NEQ; ++e) acc[e] = 0.0;
@@ -219,7 +200,7 @@ __global__ void __launch_bounds__(RolesCfg<NF, TY>::THREADS, 1)
                     for (int e = 0; e < NEQ; ++e) prefetch_l2(o.qn + (long long)e * g.cells + cell + g.sz);
                 }
             };
-            inplane_xy<D, NF, TY, ORDER, false, NT>(b ? B1 : B0, eos, cx, cy, acc, early, NoHook());
+            inplane_xy<D, NF, TY, ORDER, false, NT, MFC_ROLES_XPRE, MFC_ROLES_RIMBAL>(b ? B1 : B0, eos, cx, cy, acc, early, NoHook());
             // ---- bottom: q_s (L2: this block read the cell as a raw row three planes ago) and q_n loaded now, used last ----
             double qsv[NEQ], qnv[NEQ];
             if (active) {
@@ -232,18 +213,14 @@ __global__ void __launch_bounds__(RolesCfg<NF, TY>::THREADS, 1)
                     for (int e = 0; e < NEQ; ++e) qnv[e] = __ldcg(o.qn + (long long)e * g.cells + cell);
                 }
             }
-            if (u + 1 < U) {                                        // halo of the next staged plane: primitives in place
-                RWAIT(bars + R::FULL_P + (b ^ 1), par((u + 1) >> 1));
-                convert_halo(sm + (b ^ 1) * R::nPb);
-            }
             // ---- a4 + a5: out = ca q_n + cb q_s + coef (Lx / dx + Ly / dy + Lz / dz) ----
-            RWAIT(bars + R::FULL_LZ + b, par(u >> 1));
+            RWAIT(bars + R::FULL_LZ + lzb(u), par(lzk(u)));
             {
-                const double *const Lz = sm + R::oLz + b * R::nL;
+                const double *const Lz = sm + R::oLz + lzb(u) * R::nL;
 #pragma unroll
                 for (int e = 0; e < NEQ; ++e) acc[e] = fma(cz, Lz[e * NT + tid], acc[e]);
             }
-            warp_arrive(bars + R::EMPTY_LZ + b, lane);
+            warp_arrive(bars + R::EMPTY_LZ + lzb(u), lane);
             if (active) {
 #pragma unroll
                 for (int e = 0; e < NEQ; ++e) {
@@ -253,8 +230,7 @@ __global__ void __launch_bounds__(RolesCfg<NF, TY>::THREADS, 1)
                     o.out[(long long)e * g.cells + cell] = a;
                 }
             }
-            fence_async_proxy();                                    // this thread's writes to the next plane / reads of this one, before the box
-            inplane_sync<NT>();                                     // plane u has been read by everybody; the halo of plane u + 1 is converted
+            inplane_sync<NT>();                                     // plane u has been read by everybody
             if (tid == 0 && u + 2 < U) load_plane(u + 2);
         }
     } else {
@@ -268,8 +244,8 @@ __global__ void __launch_bounds__(RolesCfg<NF, TY>::THREADS, 1)
         for (int n = 0; n < U + 2 * NG; ++n) {
             const int u = n - 2 * NG;                               // plane whose z difference is formed (if >= 0)
             const int v = n - 2 * NG + 1;                           // plane m - 2: reconstructed along z; own cells -> staged plane
-            double *const Lz = sm + R::oLz + (u & 1) * R::nL;
-            if (u >= 2) RWAIT(bars + R::EMPTY_LZ + (u & 1), par((u - 2) >> 1));
+            double *const Lz = sm + R::oLz + lzb(u) * R::nL;
+            if (u >= R::NLZ) RWAIT(bars + R::EMPTY_LZ + lzb(u), par(lzk(u - R::NLZ)));
 #pragma unroll 1
             for (int r = 0; r < R::ZR; ++r) {
                 const int row = R::ZR * zw + r;
@@ -345,7 +321,7 @@ __global__ void __launch_bounds__(RolesCfg<NF, TY>::THREADS, 1)
                     tmem_store<TV>(trow + R::T_RING + (unsigned)((n & 3) * 2 * TV), wn);
                 }
             }
-            if (u >= 0) warp_arrive(bars + R::FULL_LZ + (u & 1), lane);
+            if (u >= 0) warp_arrive(bars + R::FULL_LZ + lzb(u), lane);
             // own cells of plane v (ring slot of plane m - 2) -> staged plane
             if (v >= 0 && v < U) {
                 double *const Pb = sm + (v & 1) * R::nPb;
@@ -358,6 +334,23 @@ __global__ void __launch_bounds__(RolesCfg<NF, TY>::THREADS, 1)
                     tmem_load<TV>(trow + R::T_RING + (unsigned)(((n + 2) & 3) * 2 * TV), w);
 #pragma unroll
                     for (int e = 0; e < NEQ; ++e) Pb[e * PPL + POWN + row * FPX + lane] = w[e];
+                }
+                // halo cells of the landed plane: raw q -> primitives in place, dealt to the Z warps in rounds of 32
+#pragma unroll 1
+                for (int h = 32 * zw + lane; h < NH; h += 32 * R::NZ) {
+                    constexpr int TOP = NG * FPX;                   // (row-major numbering of the staged plane that skips the interior block)
+                    int c;
+                    if (h < TOP) c = h;
+                    else if (h < TOP + 2 * NG * TY) {
+                        const int rr = (h - TOP) / (2 * NG), kk = (h - TOP) - rr * 2 * NG;
+                        c = (NG + rr) * FPX + (kk < NG ? kk : FTX + kk);
+                    } else c = (NG + TY) * FPX + (h - TOP - 2 * NG * TY);
+                    double qc[NEQ], wc[NEQ];
+#pragma unroll
+                    for (int e = 0; e < NEQ; ++e) qc[e] = Pb[e * PPL + c];
+                    cons_to_prim_cell<D, NF>(qc, eos, wc);
+#pragma unroll
+                    for (int e = 0; e < NEQ; ++e) Pb[e * PPL + c] = wc[e];
                 }
                 fence_async_proxy();                                // these writes precede the box that will overwrite the plane
                 warp_arrive(bars + R::PRIM_P + (v & 1), lane);

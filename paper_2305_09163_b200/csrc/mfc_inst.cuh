@@ -13,6 +13,10 @@
 #ifndef MFC_TY_2F
 #define MFC_TY_2F 12
 #endif
+// rows of the tile of the kernel with specialised Z warps (mfc_fused_roles.cuh)
+#ifndef MFC_ROLES_TY
+#define MFC_ROLES_TY 12
+#endif
 #define MFC_CAT2(a, b) a##b
 #define MFC_CAT(a, b) MFC_CAT2(a, b)
 
@@ -123,15 +127,18 @@ static cudaError_t launch_fused_nu(const typename GeoOf<NU>::type &g, const Eos 
         const bool tma_ok = path != MFC_PATH_LDGSTS && (g.p[0] & 1) == 0 && (reinterpret_cast<unsigned long long>(q) & 15) == 0 &&
                             (o.nbase == 0 || o.qs == q);
         CUtensorMap tm_plane, tm_col;
-        // warp-specialised kernel (mfc_fused_roles.cuh): uniform grid, two fluids, the TMA layout conditions
-        if constexpr (!NU && NF == 2 && TY == 12) {
+        // kernel with the z direction on specialised warps (mfc_fused_roles.cuh): uniform grid, two fluids, TMA layout conditions
+        if constexpr (!NU && NF == 2) {
             if (path == MFC_PATH_ROLES) {
-                using R = RolesCfg<NF, TY>;
-                static_assert(R::bytes <= 227 * 1024, "role-split tile does not fit shared memory");
-                if (!tma_ok || !encode_state_map(&tm_plane, g, C::NEQ, q, FPX, C::PY) || !encode_state_map(&tm_col, g, C::NEQ, q, R::CW, 1))
+                constexpr int RTY = MFC_ROLES_TY;
+                using R = RolesCfg<NF, RTY>;
+                const int rnty = (g.n[1] + RTY - 1) / RTY;
+                const int rseg = fused_segment(g, (long long)ntx * rnty, segment);
+                const unsigned rblocks = (unsigned)((long long)ntx * rnty * ((g.n[2] + rseg - 1) / rseg));
+                if (!tma_ok || !encode_state_map(&tm_plane, g, C::NEQ, q, FPX, RTY + 2 * NG) || !encode_state_map(&tm_col, g, C::NEQ, q, R::CW, 1))
                     return cudaErrorInvalidValue;
-                if ((st = MFC_OPTIN_SHARED((rhs_fused_roles_kernel<NF, TY, ORDER>), R::bytes)) != cudaSuccess) return st;
-                rhs_fused_roles_kernel<NF, TY, ORDER><<<blocks, R::THREADS, R::bytes, s>>>(tm_plane, tm_col, g, e, o, ntx, nty, seg);
+                if ((st = MFC_OPTIN_SHARED((rhs_fused_roles_kernel<NF, RTY, ORDER>), R::bytes)) != cudaSuccess) return st;
+                rhs_fused_roles_kernel<NF, RTY, ORDER><<<rblocks, R::THREADS, R::bytes, s>>>(tm_plane, tm_col, g, e, o, ntx, rnty, rseg);
                 return cudaSuccess;
             }
         } else if (path == MFC_PATH_ROLES) return cudaErrorInvalidValue;
