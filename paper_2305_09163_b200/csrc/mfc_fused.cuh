@@ -120,33 +120,21 @@ __device__ __forceinline__ void inplane_sync()
     else asm volatile("bar.sync 1, %0;" ::"n"(GT) : "memory");
 }
 
-// XP: variables whose x reconstruction runs before barrier S1; RIMBAL: the two warps that solve the rim faces between S1 and
-// S2 reconstruct one more variable before S1 than the others (their extra Riemann solve no longer delays S2 for everybody)
-template <int D, int NF, int TY, int ORDER, bool NU = false, int GT = 0, int XP = MFC_XPRE, bool RIMBAL = false, class Early = NoHook, class Mid = NoHook>
-__device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, const Eos &eos, double cx, double cy,
-                                           double (&acc)[2 * NF + D], Early early = Early(), Mid mid = Mid(),
-                                           const NuPlane &nup = NuPlane{nullptr, nullptr, 0, 0})
+// ---- rim states.  A unit = ONE variable of one rim cell, one SIDE: (kind, variable e, index r along the rim) with
+//   kind 0: left state of y face -1/2 (from row -1)          kind 1: right state of the y face past the tile (row TY)
+//   kind 2: left state of x face -1/2 (from cell -1)         kind 3: right state of the x face past the tile (cell FTX)
+//   kind 4: right state of x face -1/2 (from cell 0: recomputed here so that the rim face can be solved before lane 0
+//           publishes it)
+// dealt round-robin to ALL threads (two rounds in 3D with two fluids, the second one leaving out the two warps that
+// solve the rim faces), so that no warp reaches the barrier much later than the others.  A right state is the
+// left state of the mirrored stencil: one code path, the side only flips the sign of the stride. ----
+template <int D, int NF, int TY, int ORDER, bool NU>
+__device__ __forceinline__ void rim_units(const InplaneBufs<D, NF, TY> &B, const Eos &eos, const NuPlane &nup)
 {
     using C = FusedCfg<D, NF, TY>;
-    using I = Idx<D, NF>;
     constexpr int NEQ = C::NEQ, NT = C::NT, PPL = C::PPL, HY = C::HY;
-    constexpr int RIMW = TY - 1;                                    // warp that solves the y rim faces
-    constexpr int RIMX = TY >= 2 ? TY - 2 : 0;                      // warp that solves the x rim faces
-    const int tid = threadIdx.x, i = tid & 31, j = tid >> 5;
+    const int tid = threadIdx.x;
     const double *const P = B.P;
-    const double *const pc = P + (j + HY) * FPX + (i + NG);         // this thread's cell
-    double *const FxH = B.HxL;                                      // [NEQ+1][TY]  flux of face -1/2, over HxL, ExR[0]
-    double *const FyH = B.HyL;                                      // [NEQ+1][FTX] over HyL, HyR[0]
-
-    early();
-    // ---- rim states.  A unit = ONE variable of one rim cell, one SIDE: (kind, variable e, index r along the rim) with
-    //   kind 0: left state of y face -1/2 (from row -1)          kind 1: right state of the y face past the tile (row TY)
-    //   kind 2: left state of x face -1/2 (from cell -1)         kind 3: right state of the x face past the tile (cell FTX)
-    //   kind 4: right state of x face -1/2 (from cell 0: recomputed here so that the rim face can be solved before lane 0
-    //           publishes it)
-    // dealt round-robin to ALL threads (two rounds in 3D with two fluids, the second one leaving out the two warps that
-    // solve the rim faces below), so that no warp reaches the barrier much later than the others.  A right state is the
-    // left state of the mirrored stencil: one code path, the side only flips the sign of the stride. ----
     {
         constexpr int UY = D >= 2 ? 2 * FTX * NEQ : 0, UX = 3 * TY * NEQ, U = UY + UX;
 #pragma unroll
@@ -186,6 +174,57 @@ __device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, cons
             }
         }
     }
+}
+
+// the rim faces j = -1/2 (one warp) and i = -1/2 (TY lanes of one warp); the fluxes overwrite the left rim states
+template <int D, int NF, int TY>
+__device__ __forceinline__ void rim_face_y(const InplaneBufs<D, NF, TY> &B, const Eos &eos)
+{
+    constexpr int NEQ = 2 * NF + D, NT = FTX * TY;
+    const int i = threadIdx.x & 31;
+    double *const FyH = B.HyL;
+    double hl[NEQ], hr[NEQ], F[NEQ], uf;
+#pragma unroll
+    for (int e = 0; e < NEQ; ++e) { hl[e] = B.HyL[e * FTX + i]; hr[e] = B.X[e * NT + i]; }
+    hllc<D, NF, 1>(hl, hr, eos, F, uf);
+#pragma unroll
+    for (int e = 0; e < NEQ; ++e) FyH[e * FTX + i] = F[e];
+    FyH[NEQ * FTX + i] = uf;
+}
+template <int D, int NF, int TY>
+__device__ __forceinline__ void rim_face_x(const InplaneBufs<D, NF, TY> &B, const Eos &eos)
+{
+    constexpr int NEQ = 2 * NF + D;
+    const int i = threadIdx.x & 31;
+    double *const FxH = B.HxL;
+    double hl[NEQ], hr[NEQ], F[NEQ], uf;
+#pragma unroll
+    for (int e = 0; e < NEQ; ++e) { hl[e] = B.HxL[e * TY + i]; hr[e] = B.ExR[e * TY + i]; }
+    hllc<D, NF, 0>(hl, hr, eos, F, uf);
+#pragma unroll
+    for (int e = 0; e < NEQ; ++e) FxH[e * TY + i] = F[e];
+    FxH[NEQ * TY + i] = uf;
+}
+
+// XP: variables whose x reconstruction runs before barrier S1
+template <int D, int NF, int TY, int ORDER, bool NU = false, int GT = 0, int XP = MFC_XPRE, class Early = NoHook, class Mid = NoHook>
+__device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, const Eos &eos, double cx, double cy,
+                                           double (&acc)[2 * NF + D], Early early = Early(), Mid mid = Mid(),
+                                           const NuPlane &nup = NuPlane{nullptr, nullptr, 0, 0})
+{
+    using C = FusedCfg<D, NF, TY>;
+    using I = Idx<D, NF>;
+    constexpr int NEQ = C::NEQ, NT = C::NT, PPL = C::PPL, HY = C::HY;
+    constexpr int RIMW = TY - 1;                                    // warp that solves the y rim faces
+    constexpr int RIMX = TY >= 2 ? TY - 2 : 0;                      // warp that solves the x rim faces
+    const int tid = threadIdx.x, i = tid & 31, j = tid >> 5;
+    const double *const P = B.P;
+    const double *const pc = P + (j + HY) * FPX + (i + NG);         // this thread's cell
+    double *const FxH = B.HxL;                                      // [NEQ+1][TY]  flux of face -1/2, over HxL, ExR[0]
+    double *const FyH = B.HyL;                                      // [NEQ+1][FTX] over HyL, HyR[0]
+
+    early();
+    rim_units<D, NF, TY, ORDER, NU>(B, eos, nup);
 
     // ---- y, first half: reconstruct, publish the right state ----
     double vLy[NEQ];
@@ -203,17 +242,11 @@ __device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, cons
     // the x reconstruction needs nothing of the other warps: it runs BEFORE the barrier for the first XPRE variables,
     // so that the barrier's skew and the burst of stencil loads behind it are covered by arithmetic
     constexpr int XPRE = NEQ < XP ? NEQ : XP;
-    const bool rim_early = RIMBAL && XPRE < NEQ && (j == RIMW || j == RIMX);
     double vL[NEQ], vR[NEQ];
 #pragma unroll
     for (int e = 0; e < XPRE; ++e) {
         const double *s5 = pc + e * PPL;
         reconstruct<ORDER, NU>(s5[0], s5[-1] - s5[-2], s5[0] - s5[-1], s5[1] - s5[0], s5[2] - s5[1], eos.weno_eps4, vL[e], vR[e], NuRef{nup.tx + i, nup.sx});
-    }
-    if (rim_early) {
-        const double *s5 = pc + XPRE * PPL;
-        reconstruct<ORDER, NU>(s5[0], s5[-1] - s5[-2], s5[0] - s5[-1], s5[1] - s5[0], s5[2] - s5[1], eos.weno_eps4, vL[XPRE < NEQ ? XPRE : 0], vR[XPRE < NEQ ? XPRE : 0],
-                               NuRef{nup.tx + i, nup.sx});
     }
     inplane_sync<GT>();                                             // S1: rim states and y right states are visible
 
@@ -223,7 +256,6 @@ __device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, cons
     {
 #pragma unroll
         for (int e = XPRE; e < NEQ; ++e) {
-            if (e == XPRE && rim_early) continue;
             const double *s5 = pc + e * PPL;
             reconstruct<ORDER, NU>(s5[0], s5[-1] - s5[-2], s5[0] - s5[-1], s5[1] - s5[0], s5[2] - s5[1], eos.weno_eps4, vL[e], vR[e], NuRef{nup.tx + i, nup.sx});
         }
@@ -255,25 +287,9 @@ __device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, cons
 #pragma unroll
         for (int e = 0; e < NEQ; ++e) vRn[e] = j == TY - 1 ? B.HyR[e * FTX + i] : B.X[e * NT + tid + FTX];
         hllc<D, NF, 1>(vLy, vRn, eos, Fy, ufy);
-        if (j == RIMW) {
-            double hl[NEQ], hr[NEQ], F[NEQ], uf;
-#pragma unroll
-            for (int e = 0; e < NEQ; ++e) { hl[e] = B.HyL[e * FTX + i]; hr[e] = B.X[e * NT + i]; }
-            hllc<D, NF, 1>(hl, hr, eos, F, uf);
-#pragma unroll
-            for (int e = 0; e < NEQ; ++e) FyH[e * FTX + i] = F[e];
-            FyH[NEQ * FTX + i] = uf;
-        }
+        if (j == RIMW) rim_face_y<D, NF, TY>(B, eos);
     }
-    if (j == RIMX && i < TY) {                                      // rim faces i = -1/2, one per row
-        double hl[NEQ], hr[NEQ], F[NEQ], uf;
-#pragma unroll
-        for (int e = 0; e < NEQ; ++e) { hl[e] = B.HxL[e * TY + i]; hr[e] = B.ExR[e * TY + i]; }
-        hllc<D, NF, 0>(hl, hr, eos, F, uf);
-#pragma unroll
-        for (int e = 0; e < NEQ; ++e) FxH[e * TY + i] = F[e];
-        FxH[NEQ * TY + i] = uf;
-    }
+    if (j == RIMX && i < TY) rim_face_x<D, NF, TY>(B, eos);                 // rim faces i = -1/2, one per row
     if constexpr (D >= 2) {                                         // the fluxes have a buffer of their own: no barrier before this
 #pragma unroll
         for (int e = 0; e < NEQ; ++e) B.X2[e * NT + tid] = Fy[e];

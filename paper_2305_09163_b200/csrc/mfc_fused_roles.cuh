@@ -21,9 +21,6 @@
 #ifndef MFC_ROLES_XPRE
 #define MFC_ROLES_XPRE 4    // x reconstructions before barrier S1 (0 .. 7: 2.380 2.355 2.385 2.361 2.353 . . 2.414 ms at cfg3)
 #endif
-#ifndef MFC_ROLES_RIMBAL
-#define MFC_ROLES_RIMBAL false
-#endif
 
 namespace mfc {
 
@@ -200,7 +197,7 @@ __global__ void __launch_bounds__(RolesCfg<NF, TY>::THREADS, 1)
                     for (int e = 0; e < NEQ; ++e) prefetch_l2(o.qn + (long long)e * g.cells + cell + g.sz);
                 }
             };
-            inplane_xy<D, NF, TY, ORDER, false, NT, MFC_ROLES_XPRE, MFC_ROLES_RIMBAL>(b ? B1 : B0, eos, cx, cy, acc, early, NoHook());
+            inplane_xy<D, NF, TY, ORDER, false, NT, MFC_ROLES_XPRE>(b ? B1 : B0, eos, cx, cy, acc, early, NoHook());
             // ---- bottom: q_s (L2: this block read the cell as a raw row three planes ago) and q_n loaded now, used last ----
             double qsv[NEQ], qnv[NEQ];
             if (active) {

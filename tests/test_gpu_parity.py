@@ -236,6 +236,59 @@ def test_tma_staging_refuses_an_odd_padded_extent_and_auto_falls_back():
     check_rhs(prob, q, staging=B.MFC_STAGING_AUTO)
 
 
+# ---------------------------------------------------------------------------------------------
+# the 3D kernel with specialised Z warps (staging = 3; what AUTO runs for two fluids on a uniform grid
+# with an even padded extent): forced, against the oracle and against the one-loop kernel
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("periodic", [True, False])
+@pytest.mark.parametrize("order", [5, 3, 1])
+@pytest.mark.parametrize("n,seg", [((70, 29, 41), 8), ((32, 12, 9), 0), ((96, 50, 7), 3), ((34, 13, 64), 0)])
+def test_rhs_parity_split_kernel(periodic, order, n, seg):
+    """Ragged tiles in x and y (rows past the domain in the last tile row), one to many z segments, segments of a single
+    plane; every reconstruction order.  The split kernel sums the three directions in another order than the one-loop
+    kernel, so the two are compared at round-off, not bitwise."""
+    import dataclasses
+    prob, q = wl.random_state(3, n, 2, seed=400 + order, periodic=periodic)
+    prob = dataclasses.replace(prob, weno_order=order)
+    check_rhs(prob, q, march_segment=seg, staging=B.MFC_STAGING_ROLES)
+    with Gpu(prob, march_segment=seg, staging=B.MFC_STAGING_ROLES) as g1, Gpu(prob, march_segment=seg, staging=B.MFC_STAGING_TMA) as g2:
+        it = prob.interior()
+        a, b = g1.rhs(q)[it], g2.rhs(q)[it]
+        scale = np.max(np.abs(b), axis=(1, 2, 3), keepdims=True) + 1e-300
+        assert np.max(np.abs(a - b) / scale) <= 1e-12
+
+
+@pytest.mark.parametrize("rough", [False, True])
+@pytest.mark.parametrize("kapila", [False, True])
+def test_rk3_parity_split_kernel(rough, kapila):
+    import dataclasses
+    prob, q = wl.random_state(3, (40, 30, 33), 2, seed=410, periodic=not rough, rough=rough)
+    prob = dataclasses.replace(prob, kapila=kapila)
+    check_rk(prob, q, march_segment=8, staging=B.MFC_STAGING_ROLES)
+
+
+def test_split_kernel_is_reproducible_and_refuses_what_it_does_not_cover():
+    """Run-to-run bitwise reproducibility (a race between the warp kinds would show here), and a forced choice fails for three
+    fluids, for an odd padded extent and on a stretched grid while AUTO falls back to a kernel that applies."""
+    prob, q = wl.random_state(3, (64, 24, 40), 2, seed=411, periodic=False)
+    with Gpu(prob, staging=B.MFC_STAGING_ROLES) as g:
+        ref = g.rhs(q)
+        for _ in range(5):
+            assert np.array_equal(g.rhs(q), ref, equal_nan=True)
+    for p3, q3 in (wl.random_state(3, (40, 17, 9), 3, seed=5, periodic=True, rough=False),
+                   wl.random_state(3, (33, 17, 9), 2, seed=5, periodic=True, rough=False)):
+        with Gpu(p3, staging=B.MFC_STAGING_ROLES) as g:
+            with pytest.raises(B.MfcError):
+                g.rhs(q3)
+        check_rhs(p3, q3, staging=B.MFC_STAGING_AUTO)
+    ps, qs = wl.random_state(3, (40, 17, 12), 2, seed=6, periodic=False, rough=False)
+    ps = wl.with_stretched_grid(ps)
+    with Gpu(ps, staging=B.MFC_STAGING_ROLES) as g:
+        with pytest.raises(B.MfcError):
+            g.rhs(qs)
+    check_rhs(ps, qs, staging=B.MFC_STAGING_AUTO)
+
+
 @pytest.mark.parametrize("seg", [1, 5, 32, 1000])
 @pytest.mark.parametrize("n0", [40, 41])
 def test_rhs_is_independent_of_the_marching_segment(seg, n0):
