@@ -1,4 +1,4 @@
-// The 3D right-hand side with the z direction split off to SPECIALISED warps (uniform grid):
+// The 3D right-hand side with the z direction split off to SPECIALISED warps (uniform grid, any number of fluids):
 // same decomposition as rhs_fused_march_tma_kernel (tile of 32 x TY cells in (x, y), march along z three planes ahead,
 // TMA-staged planes, z window in tensor memory), but the block has two kinds of warps, each with a loop of its own:
 //   in-plane warps (TY, one row each): the x and y differences of the staged plane (inplane_xy, mfc_fused.cuh, its two
@@ -97,7 +97,7 @@ struct RolesCfg {
     static constexpr int oX2 = oX + NEQ * NT;                            //             fluxes [NEQ][NT]
     static constexpr int nL = NEQ * NT;
     static constexpr int oLz = r16(oX2 + NEQ * NT);                      // z flux differences [2][NEQ][NT]
-    static constexpr int NLZ = TY > 12 ? 1 : 2;
+    static constexpr int NLZ = (TY > 12 || NEQ > 7) ? 1 : 2;               // (one buffer where two do not fit shared memory)
     static constexpr int oBar = oLz + NLZ * nL;
     enum { FULL_P = 0, PRIM_P = 2, FULL_LZ = 4, EMPTY_LZ = 6, FULL_SQ = 8, NBAR = FULL_SQ + TY, TMEM_WORD = NBAR, NWORDS = NBAR + 1 };
     static constexpr int doubles = oBar + r16(NWORDS);

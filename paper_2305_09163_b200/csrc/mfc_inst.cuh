@@ -127,9 +127,9 @@ static cudaError_t launch_fused_nu(const typename GeoOf<NU>::type &g, const Eos 
         const bool tma_ok = path != MFC_PATH_LDGSTS && (g.p[0] & 1) == 0 && (reinterpret_cast<unsigned long long>(q) & 15) == 0 &&
                             (o.nbase == 0 || o.qs == q);
         CUtensorMap tm_plane, tm_col;
-        // kernel with the z direction on specialised warps (mfc_fused_roles.cuh): uniform grid, two fluids, the TMA layout
-        // conditions; AUTO prefers it where it applies (2.31 against 2.55 ms per evaluation at 256^3)
-        if constexpr (!NU && NF == 2) {
+        // kernel with the z direction on specialised warps (mfc_fused_roles.cuh): uniform grid, the TMA layout conditions;
+        // AUTO prefers it where it applies (256^3, two fluids: 2.31 against 2.55 ms per evaluation; 384^3, three: 9.9 against 11.7)
+        if constexpr (!NU) {
             if ((path == MFC_PATH_ROLES || path == MFC_PATH_AUTO) && tma_ok) {
                 constexpr int RTY = MFC_ROLES_TY;
                 using R = RolesCfg<NF, RTY>;

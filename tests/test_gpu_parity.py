@@ -258,6 +258,15 @@ def test_rhs_parity_split_kernel(periodic, order, n, seg):
         assert np.max(np.abs(a - b) / scale) <= 1e-12
 
 
+@pytest.mark.parametrize("nf", [1, 3])
+@pytest.mark.parametrize("periodic", [True, False])
+def test_rhs_and_rk3_parity_split_kernel_one_and_three_fluids(nf, periodic):
+    prob, q = wl.random_state(3, (70, 29, 41), nf, seed=420 + nf, periodic=periodic)
+    check_rhs(prob, q, march_segment=8, staging=B.MFC_STAGING_ROLES)
+    prob, q = wl.random_state(3, (40, 30, 33), nf, seed=430 + nf, periodic=periodic, rough=False)
+    check_rk(prob, q, march_segment=8, staging=B.MFC_STAGING_ROLES)
+
+
 @pytest.mark.parametrize("rough", [False, True])
 @pytest.mark.parametrize("kapila", [False, True])
 def test_rk3_parity_split_kernel(rough, kapila):
@@ -268,19 +277,18 @@ def test_rk3_parity_split_kernel(rough, kapila):
 
 
 def test_split_kernel_is_reproducible_and_refuses_what_it_does_not_cover():
-    """Run-to-run bitwise reproducibility (a race between the warp kinds would show here), and a forced choice fails for three
-    fluids, for an odd padded extent and on a stretched grid while AUTO falls back to a kernel that applies."""
+    """Run-to-run bitwise reproducibility (a race between the warp kinds would show here), and a forced choice fails for an
+    odd padded extent and on a stretched grid while AUTO falls back to a kernel that applies."""
     prob, q = wl.random_state(3, (64, 24, 40), 2, seed=411, periodic=False)
     with Gpu(prob, staging=B.MFC_STAGING_ROLES) as g:
         ref = g.rhs(q)
         for _ in range(5):
             assert np.array_equal(g.rhs(q), ref, equal_nan=True)
-    for p3, q3 in (wl.random_state(3, (40, 17, 9), 3, seed=5, periodic=True, rough=False),
-                   wl.random_state(3, (33, 17, 9), 2, seed=5, periodic=True, rough=False)):
-        with Gpu(p3, staging=B.MFC_STAGING_ROLES) as g:
-            with pytest.raises(B.MfcError):
-                g.rhs(q3)
-        check_rhs(p3, q3, staging=B.MFC_STAGING_AUTO)
+    p3, q3 = wl.random_state(3, (33, 17, 9), 2, seed=5, periodic=True, rough=False)
+    with Gpu(p3, staging=B.MFC_STAGING_ROLES) as g:
+        with pytest.raises(B.MfcError):
+            g.rhs(q3)
+    check_rhs(p3, q3, staging=B.MFC_STAGING_AUTO)
     ps, qs = wl.random_state(3, (40, 17, 12), 2, seed=6, periodic=False, rough=False)
     ps = wl.with_stretched_grid(ps)
     with Gpu(ps, staging=B.MFC_STAGING_ROLES) as g:
