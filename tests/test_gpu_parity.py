@@ -258,6 +258,16 @@ def test_rhs_parity_split_kernel(periodic, order, n, seg):
         assert np.max(np.abs(a - b) / scale) <= 1e-12
 
 
+@pytest.mark.parametrize("n", [(4, 3, 3), (4, 4, 4), (6, 3, 5), (34, 3, 3), (4, 13, 3), (4, 3, 14), (32, 12, 3)])
+@pytest.mark.parametrize("periodic", [True, False])
+def test_rhs_parity_split_kernel_smallest_grids(n, periodic):
+    """Degenerate sizes: fewer cells than ghost layers + 1 per dimension, one tile with most of its rows and lanes past the
+    domain, segments shorter than the three planes the z direction runs ahead."""
+    prob, q = wl.random_state(3, n, 2, seed=440, periodic=periodic, rough=False)
+    check_rhs(prob, q, staging=B.MFC_STAGING_ROLES)
+    check_rhs(prob, q, march_segment=1, staging=B.MFC_STAGING_ROLES)
+
+
 @pytest.mark.parametrize("nf", [1, 3])
 @pytest.mark.parametrize("periodic", [True, False])
 def test_rhs_and_rk3_parity_split_kernel_one_and_three_fluids(nf, periodic):
