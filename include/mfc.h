@@ -96,7 +96,7 @@ typedef struct {
                           (PAPER.md:52, 60-62), cell-centred, on the same face-velocity differences as alpha div(u);
                           needs n_fluids == 2 and volume fractions inside (0, 1).  0: Allaire model, K = 0 */
     int staging;       /* which 3D kernel runs: 0 = automatic: the kernel with specialised Z warps (TMA-staged;
-                          uniform spacing, even padded extent in x (n[0] even) and a 16-byte aligned q_dev), else the one-loop
+                          even padded extent in x (n[0] even) and a 16-byte aligned q_dev), else the one-loop
                           kernel staged by TMA boxes (same layout conditions), else the one-loop kernel staged by per-thread
                           cp.async; 1 = one-loop kernel, TMA only; 2 = one-loop kernel, cp.async only; 3 = specialised Z
                           warps only.  A forced choice fails with MFC_ECUDA where it does not apply.  The one-loop kernels

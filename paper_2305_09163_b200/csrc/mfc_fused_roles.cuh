@@ -1,4 +1,4 @@
-// The 3D right-hand side with the z direction split off to SPECIALISED warps (uniform grid, any number of fluids):
+// The 3D right-hand side with the z direction split off to SPECIALISED warps (any number of fluids; uniform grid or per-index tables):
 // same decomposition as rhs_fused_march_tma_kernel (tile of 32 x TY cells in (x, y), march along z three planes ahead,
 // TMA-staged planes, z window in tensor memory), but the block has two kinds of warps, each with a loop of its own:
 //   in-plane warps (TY, one row each): the x and y differences of the staged plane (inplane_xy, mfc_fused.cuh, its two
@@ -114,10 +114,10 @@ struct RolesCfg {
     static_assert(2 * bytes > 227 * 1024, "two resident blocks would deadlock in tcgen05.alloc");
 };
 
-template <int NF, int TY, int ORDER>
+template <int NF, int TY, int ORDER, bool NU>
 __global__ void __launch_bounds__(RolesCfg<NF, TY>::THREADS, 1)
-    rhs_fused_roles_kernel(const __grid_constant__ CUtensorMap tm_plane, const __grid_constant__ CUtensorMap tm_col, Geo g, Eos eos, SweepOut o,
-                           int ntx, int nty, int seg)
+    rhs_fused_roles_kernel(const __grid_constant__ CUtensorMap tm_plane, const __grid_constant__ CUtensorMap tm_col, typename GeoOf<NU>::type g, Eos eos,
+                           SweepOut o, int ntx, int nty, int seg)
 {
     constexpr int D = 3;
     using R = RolesCfg<NF, TY>;
@@ -167,6 +167,7 @@ __global__ void __launch_bounds__(RolesCfg<NF, TY>::THREADS, 1)
         mbar_expect_tx(bars + R::FULL_SQ + row, R::row_bytes);
         tma_load_4d(SQ + row * R::nSQr, &tm_col, bars + R::FULL_SQ + row, x0 + NG - 1, y0 + NG + row, k0 + n, 0);
     };
+
     const double cz = o.coef * g.inv_dx[2];
 
     if (warp < TY) {
@@ -186,7 +187,12 @@ __global__ void __launch_bounds__(RolesCfg<NF, TY>::THREADS, 1)
             const long long cell = (long long)(k0 + u + NG) * g.sz + col;
             double coef = o.coef;
             asm volatile("" : "+d"(coef));
-            const double cx = coef * g.inv_dx[0], cy = coef * g.inv_dx[1];
+            double cx = coef * g.inv_dx[0], cy = coef * g.inv_dx[1], czp = cz;
+            if constexpr (NU) {                                     // the cell's own widths (Eq. 8-9): entry 27 of the tables
+                cx = coef * __ldg(g.nu[0] + x0 + NG + i + 27 * g.nus[0]);
+                cy = coef * __ldg(g.nu[1] + y0 + NG + j + 27 * g.nus[1]);
+                czp = coef * __ldg(g.nu[2] + k0 + u + NG + 27 * g.nus[2]);
+            }
             RWAIT(bars + R::PRIM_P + b, par(u >> 1));                  // the Z warps have made plane u primitives (own cells and halo)
             double acc[NEQ];
 #pragma unroll
@@ -197,7 +203,12 @@ __global__ void __launch_bounds__(RolesCfg<NF, TY>::THREADS, 1)
                     for (int e = 0; e < NEQ; ++e) prefetch_l2(o.qn + (long long)e * g.cells + cell + g.sz);
                 }
             };
-            inplane_xy<D, NF, TY, ORDER, false, NT, MFC_ROLES_XPRE>(b ? B1 : B0, eos, cx, cy, acc, early, NoHook());
+            if constexpr (NU) {                                     // per-index coefficient tables of the tile's columns and rows
+                inplane_xy<D, NF, TY, ORDER, true, NT, MFC_ROLES_XPRE>(b ? B1 : B0, eos, cx, cy, acc, early, NoHook(),
+                                                                       NuPlane{g.nu[0] + x0 + NG, g.nu[1] + y0 + NG, g.nus[0], g.nus[1]});
+            } else {
+                inplane_xy<D, NF, TY, ORDER, false, NT, MFC_ROLES_XPRE>(b ? B1 : B0, eos, cx, cy, acc, early, NoHook());
+            }
             // ---- bottom: q_s (L2: this block read the cell as a raw row three planes ago) and q_n loaded now, used last ----
             double qsv[NEQ], qnv[NEQ];
             if (active) {
@@ -215,7 +226,7 @@ __global__ void __launch_bounds__(RolesCfg<NF, TY>::THREADS, 1)
             {
                 const double *const Lz = sm + R::oLz + lzb(u) * R::nL;
 #pragma unroll
-                for (int e = 0; e < NEQ; ++e) acc[e] = fma(cz, Lz[e * NT + tid], acc[e]);
+                for (int e = 0; e < NEQ; ++e) acc[e] = fma(czp, Lz[e * NT + tid], acc[e]);
             }
             warp_arrive(bars + R::EMPTY_LZ + lzb(u), lane);
             if (active) {
@@ -265,6 +276,8 @@ __global__ void __launch_bounds__(RolesCfg<NF, TY>::THREADS, 1)
                     // window of the variables 2p, 2p + 1: planes m - 4 .. m - 1 from the ring (plane m - 4 sits in the slot
                     // plane m is about to take); reconstruct cell m - 2
                     double vLn[TV], vR[NEQ], vbE = 0.0, vbA[I::NA > 0 ? I::NA : 1];
+                    NuRef nz{nullptr, 0};
+                    if constexpr (NU) nz = NuRef{g.nu[2] + k0 + v + NG, g.nus[2]};     // tables of cell m - 2 = k0 + v
 #pragma unroll
                     for (int p = 0; p < (NEQ + 1) / 2; ++p) {
                         unsigned w4[4], w3[4], w2[4], w1[4];
@@ -279,7 +292,7 @@ __global__ void __launch_bounds__(RolesCfg<NF, TY>::THREADS, 1)
                             if (e < NEQ) {
                                 const double a4 = pair_double(w4[2 * h], w4[2 * h + 1]), a3 = pair_double(w3[2 * h], w3[2 * h + 1]);
                                 const double a2 = pair_double(w2[2 * h], w2[2 * h + 1]), a1 = pair_double(w1[2 * h], w1[2 * h + 1]);
-                                reconstruct<ORDER>(a2, a3 - a4, a2 - a3, a1 - a2, wn[e] - a1, eos.weno_eps4, vLn[e], vR[e]);
+                                reconstruct<ORDER, NU>(a2, a3 - a4, a2 - a3, a1 - a2, wn[e] - a1, eos.weno_eps4, vLn[e], vR[e], nz);
                                 if (e == I::E) vbE = a3;
                                 if (e >= I::A) vbA[e - I::A] = a3;
                             }

@@ -127,18 +127,19 @@ static cudaError_t launch_fused_nu(const typename GeoOf<NU>::type &g, const Eos 
         const bool tma_ok = path != MFC_PATH_LDGSTS && (g.p[0] & 1) == 0 && (reinterpret_cast<unsigned long long>(q) & 15) == 0 &&
                             (o.nbase == 0 || o.qs == q);
         CUtensorMap tm_plane, tm_col;
-        // kernel with the z direction on specialised warps (mfc_fused_roles.cuh): uniform grid, the TMA layout conditions;
+        // kernel with the z direction on specialised warps (mfc_fused_roles.cuh): the TMA layout conditions;
         // AUTO prefers it where it applies (256^3, two fluids: 2.31 against 2.55 ms per evaluation; 384^3, three: 9.9 against 11.7)
-        if constexpr (!NU) {
-            if ((path == MFC_PATH_ROLES || path == MFC_PATH_AUTO) && tma_ok) {
+        {
+            // (three fluids on a non-uniform grid: 464 B of spills in the split kernel; AUTO keeps the one-loop kernel there)
+            if ((path == MFC_PATH_ROLES || (path == MFC_PATH_AUTO && (!NU || NF <= 2))) && tma_ok) {
                 constexpr int RTY = MFC_ROLES_TY;
                 using R = RolesCfg<NF, RTY>;
                 const int rnty = (g.n[1] + RTY - 1) / RTY;
                 const int rseg = fused_segment(g, (long long)ntx * rnty, segment);
                 const unsigned rblocks = (unsigned)((long long)ntx * rnty * ((g.n[2] + rseg - 1) / rseg));
                 if (encode_state_map(&tm_plane, g, C::NEQ, q, FPX, RTY + 2 * NG) && encode_state_map(&tm_col, g, C::NEQ, q, R::CW, 1)) {
-                    if ((st = MFC_OPTIN_SHARED((rhs_fused_roles_kernel<NF, RTY, ORDER>), R::bytes)) != cudaSuccess) return st;
-                    rhs_fused_roles_kernel<NF, RTY, ORDER><<<rblocks, R::THREADS, R::bytes, s>>>(tm_plane, tm_col, g, e, o, ntx, rnty, rseg);
+                    if ((st = MFC_OPTIN_SHARED((rhs_fused_roles_kernel<NF, RTY, ORDER, NU>), R::bytes)) != cudaSuccess) return st;
+                    rhs_fused_roles_kernel<NF, RTY, ORDER, NU><<<rblocks, R::THREADS, R::bytes, s>>>(tm_plane, tm_col, g, e, o, ntx, rnty, rseg);
                     return cudaSuccess;
                 }
             }

@@ -61,8 +61,8 @@ struct SweepOut {
 };
 
 cudaError_t launch_prim(int ndim, int nf, const Geo &g, const Eos &e, const double *q, double *w, cudaStream_t s);
-// 3D kernel: AUTO = the kernel with specialised Z warps (mfc_fused_roles.cuh) where it applies (uniform grid,
-// TMA layout conditions), else the one-loop kernel staged by TMA boxes where the layout allows them (even padded extent in
+// 3D kernel: AUTO = the kernel with specialised Z warps (mfc_fused_roles.cuh) where it applies (TMA layout
+// conditions), else the one-loop kernel staged by TMA boxes where the layout allows them (even padded extent in
 // x, 16-byte aligned base), else per-thread cp.async; the other values force one of the three (and fail where it does not apply)
 enum { MFC_PATH_AUTO = 0, MFC_PATH_TMA = 1, MFC_PATH_LDGSTS = 2, MFC_PATH_ROLES = 3 };
 // g.nu[0] != nullptr selects the table-driven (non-uniform) instantiations
