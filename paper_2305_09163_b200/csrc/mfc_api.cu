@@ -63,31 +63,31 @@ cudaError_t launch_line(int ndim, int nf, int order, int dir, const Eos &e, int 
 // ---------------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) ghost_fill_kernel(Geo g, int neq, double *q)
 {
-    const long long nzs = (long long)(g.p[2] - g.n[2]) * g.p[1] * g.p[0];           // z slabs: 2 g[2] planes
-    const long long nys = (long long)g.n[2] * (g.p[1] - g.n[1]) * g.p[0];           // y slabs: 2 g[1] rows per interior plane
-    const long long nxs = (long long)g.n[2] * g.n[1] * (g.p[0] - g.n[0]);           // x slabs: 2 g[0] cells per interior row
-    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    // (32-bit index arithmetic: the shell of any array that fits the device has fewer than 2^32 cells; checked by the launcher)
+    const unsigned p0 = (unsigned)g.p[0], p1 = (unsigned)g.p[1], n1 = (unsigned)g.n[1];
+    const unsigned nzs = (unsigned)(g.p[2] - g.n[2]) * p1 * p0;                      // z slabs: 2 g[2] planes
+    const unsigned nys = (unsigned)g.n[2] * (unsigned)(g.p[1] - g.n[1]) * p0;        // y slabs: 2 g[1] rows per interior plane
+    const unsigned nxs = (unsigned)g.n[2] * n1 * (unsigned)(g.p[0] - g.n[0]);        // x slabs: 2 g[0] cells per interior row
+    const unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
     int i, j, k;
     if (t < nzs) {
-        i = (int)(t % g.p[0]);
-        const long long r = t / g.p[0];
-        j = (int)(r % g.p[1]);
-        const int kk = (int)(r / g.p[1]);
-        k = kk < g.g[2] ? kk : kk + g.n[2];
+        const unsigned r = t / p0;
+        i = (int)(t - r * p0);
+        const unsigned kk = r / p1;
+        j = (int)(r - kk * p1);
+        k = (int)kk < g.g[2] ? (int)kk : (int)kk + g.n[2];
     } else if (t < nzs + nys) {
-        const long long u = t - nzs;
-        i = (int)(u % g.p[0]);
-        const long long r = u / g.p[0];
-        const int jj = (int)(r % (2 * g.g[1]));
-        j = jj < g.g[1] ? jj : jj + g.n[1];
-        k = (int)(r / (2 * g.g[1])) + g.g[2];
+        const unsigned u = t - nzs, r = u / p0, gy2 = 2u * (unsigned)g.g[1];
+        i = (int)(u - r * p0);
+        const unsigned kk = r / gy2, jj = r - kk * gy2;
+        j = (int)jj < g.g[1] ? (int)jj : (int)jj + g.n[1];
+        k = (int)kk + g.g[2];
     } else if (t < nzs + nys + nxs) {
-        const long long u = t - nzs - nys;
-        const int ii = (int)(u % (2 * g.g[0]));
-        i = ii < g.g[0] ? ii : ii + g.n[0];
-        const long long r = u / (2 * g.g[0]);
-        j = (int)(r % g.n[1]) + g.g[1];
-        k = (int)(r / g.n[1]) + g.g[2];
+        const unsigned u = t - nzs - nys, gx2 = 2u * (unsigned)g.g[0], r = u / gx2, ii = u - r * gx2;
+        i = (int)ii < g.g[0] ? (int)ii : (int)ii + g.n[0];
+        const unsigned kk = r / n1;
+        j = (int)(r - kk * n1) + g.g[1];
+        k = (int)kk + g.g[2];
     } else return;
     const int si = bc_source(i - g.g[0], g.n[0], g.bc_lo[0], g.bc_hi[0]) + g.g[0];
     const int sj = bc_source(j - g.g[1], g.n[1], g.bc_lo[1], g.bc_hi[1]) + g.g[1];
@@ -101,6 +101,7 @@ cudaError_t launch_ghost_fill(const Geo &g, int neq, double *q, cudaStream_t s)
 {
     const long long shell = g.cells - (long long)g.n[0] * g.n[1] * g.n[2];
     if (shell <= 0) return cudaSuccess;
+    if (shell >= (1ll << 32) - 256) return cudaErrorInvalidValue;
     ghost_fill_kernel<<<(unsigned)((shell + 255) / 256), 256, 0, s>>>(g, neq, q);
     return cudaGetLastError();
 }

@@ -195,6 +195,7 @@ cudaError_t MFC_CAT(launch_cfl_d, MFC_D)(int nf, const GeoNu &g, const Eos &e, c
 {
     constexpr int D = MFC_D;
     const long long ncell = (long long)g.n[0] * g.n[1] * g.n[2];
+    if (ncell >= (1ll << 32)) return cudaErrorInvalidValue;          // (the kernel indexes cells with 32 bits; 4 G cells do not fit a B200 anyway)
     long long want = (ncell + 255) / 256;
     const unsigned blocks = (unsigned)(want < 148 * 16 ? (want < 1 ? 1 : want) : 148 * 16);
     if (g.nu[0]) { MFC_FOR_NF(nf, (cfl_kernel<D, NF, true><<<blocks, 256, 0, s>>>(g, e, q, min_bits))) }

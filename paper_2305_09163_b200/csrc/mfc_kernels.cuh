@@ -68,9 +68,11 @@ __global__ void __launch_bounds__(256) cfl_kernel(typename GeoOf<NU>::type g, Eo
     const long long stride = (long long)gridDim.x * blockDim.x;
     // cell f of the interior (x fastest): offset in the padded array and the inverse widths of the cell (Eq. 8)
     auto cell_of = [&](long long f, double (&inv)[3]) -> long long {
-        const int i = (int)(f % g.n[0]);
-        const long long r = f / g.n[0];
-        const int j = (int)(r % g.n[1]), k = (int)(r / g.n[1]);
+        // (32-bit index arithmetic: 64-bit division costs more than the rest of the cell; the launcher checks the range)
+        const unsigned fu = (unsigned)f, n0 = (unsigned)g.n[0], n1 = (unsigned)g.n[1];
+        const unsigned r = fu / n0;
+        const int i = (int)(fu - r * n0);
+        const int k = (int)(r / n1), j = (int)(r - (unsigned)k * n1);
         if constexpr (NU) {
             inv[0] = __ldg(g.nu[0] + i + NG + 27 * g.nus[0]);
             inv[1] = D > 1 ? __ldg(g.nu[1] + j + NG + 27 * g.nus[1]) : 1.0;
