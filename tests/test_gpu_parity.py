@@ -823,3 +823,20 @@ def test_dfma_probe_reports_a_plausible_fp64_rate():
     build.build()
     tf, ms = B.mfc_probe_dfma(-1)
     assert 5.0 < tf < 80.0 and ms > 0.0
+
+
+def test_long_run_stays_finite_and_is_bitwise_reproducible():
+    """150 steps (CFL + RK3 each) of the shock-bubble workload at 64^3 through the default 3D kernel, twice: finite state, the
+    same bits both times (the two warp kinds of the split kernel meet only through mbarriers; a race would show here)."""
+    prob, q = wl.cfg2(n=64)
+    outs = []
+    for _ in range(2):
+        with Gpu(prob) as g:
+            qd = g.to_dev(q)
+            for _s in range(150):
+                dt = B.mfc_cfl_dt(g.ctx, qd.data_ptr(), g.stream)
+                B.mfc_rk3_step(g.ctx, qd.data_ptr(), dt, g.stream)
+            g.torch.cuda.synchronize()
+            outs.append(qd.cpu().numpy()[prob.interior()])
+    assert np.all(np.isfinite(outs[0]))
+    assert np.array_equal(outs[0], outs[1])
