@@ -297,6 +297,117 @@ def test_hllc_alpha_flux_is_alpha_times_face_velocity():
 
 
 # ---------------------------------------------------------------------------------------------
+# A6 star state: the rows the pins above are blind to (s_* != u_K on unequal states).
+# Eq. 13-14 build q*_K so that the star flux IS the physical flux of a state moving at s_* under the
+# contact pressure p* ("u and p continuous across the contact"):
+#     F*_K = s_* q*_K + p* (0, n, s_*).
+# Two consequences that need no star-state formula:
+#   (i)  every passively carried row (alpha_i rho_i, rho u_t, alpha_i) is its upwind cell value times ONE face velocity;
+#   (ii) in the frame that moves with the contact (s_* = 0) nothing crosses the face: the mass, tangential-momentum and
+#        energy fluxes vanish and the normal-momentum flux is p*.
+# ---------------------------------------------------------------------------------------------
+def _davis_speeds(prob, direction, wL, iL, wR, iR):
+    """Reading B11: s_L = min(u_L - c_L, u_R - c_R), s_R = max(u_L + c_L, u_R + c_R)."""
+    uL, uR = wL[prob.nf + direction], wR[prob.nf + direction]
+    return min(uL - iL["c"], uR - iR["c"]), max(uL + iL["c"], uR + iR["c"])
+
+
+def _contact_speed_and_pressure(prob, direction, wL, iL, wR, iR):
+    """s_* and p* from the statement itself: the momentum jump across the outer wave of side K gives the pressure behind
+    it as a function of the contact speed s, p*_K(s) = p_K + rho_K (s_K - u_K)(s - u_K); s_* is where the two sides
+    agree.  The function is linear in s: its root follows from two evaluations (one secant step is exact)."""
+    nf, D = prob.nf, prob.ndim
+    sL, sR = _davis_speeds(prob, direction, wL, iL, wR, iR)
+    uL, uR, pL, pR = wL[nf + direction], wR[nf + direction], wL[nf + D], wR[nf + D]
+    behind_L = lambda s: pL + iL["rho"] * (sL - uL) * (s - uL)
+    behind_R = lambda s: pR + iR["rho"] * (sR - uR) * (s - uR)
+    gap = lambda s: behind_L(s) - behind_R(s)
+    s0, s1 = uL, uR if uR != uL else uL + iL["c"]
+    s_star = s0 - gap(s0) * (s1 - s0) / (gap(s1) - gap(s0))
+    return s_star, 0.5 * (behind_L(s_star) + behind_R(s_star)), sL, sR
+
+
+def _subsonic_pair(prob, rng):
+    """Unequal states a factor <= 10 apart in pressure, |u| <= 0.8 c on both sides."""
+    wL, iL = _random_prims(prob, rng, mach_max=0.8)
+    wR, iR = _random_prims(prob, rng, mach_max=0.8)
+    wR[prob.nf + prob.ndim] = wL[prob.nf + prob.ndim] * 10 ** rng.uniform(-1, 1)
+    iR["c"] = np.sqrt(((iR["Gam"] + 1) * wR[prob.nf + prob.ndim] + iR["Pi"]) / (iR["Gam"] * iR["rho"]))
+    return wL, iL, wR, iR
+
+
+@pytest.mark.parametrize("ndim,nf", [(2, 1), (2, 2), (3, 2), (3, 3)])
+def test_hllc_tangential_momentum_flux_is_upwind_momentum_times_face_velocity(ndim, nf):
+    """(i) for the rho u_t rows: F[rho u_t] = (rho u_t)_K u_face, K the side sign(s_*) selects (reading B13) -- the form
+    test_hllc_alpha_flux_is_alpha_times_face_velocity checks on the alpha and alpha_i rho_i rows only."""
+    prob, _ = wl.random_state(ndim, (4, 4, 4), nf, seed=1)
+    orc = oracle.Oracle(prob)
+    rng = np.random.default_rng(31 + 10 * ndim + nf)
+    nstar = 0
+    for _ in range(300):
+        wL, iL = _random_prims(prob, rng, mach_max=1.5)
+        wR, iR = _random_prims(prob, rng, mach_max=1.5)
+        for direction in range(ndim):
+            s_star, _, sL, sR = _contact_speed_and_pressure(prob, direction, wL, iL, wR, iR)
+            if abs(s_star) < 1e-9 * max(iL["c"], iR["c"]):
+                continue                                           # the side is not decided at round-off of s_*
+            F, uf = orc.hllc(direction, wL, wR)
+            up, iu = (wL, iL) if s_star > 0 else (wR, iR)
+            nstar += sL < 0 < sR
+            for t in range(ndim):
+                if t == direction:
+                    continue
+                mom = iu["rho"] * up[nf + t]
+                tol = 1e-12 * iu["rho"] * (abs(up[nf + t]) + 1e-3 * iu["c"]) * (abs(up[nf + direction]) + iu["c"])
+                assert abs(F[nf + t] - mom * uf) <= tol, (F[nf + t], mom * uf)
+    assert nstar > 100    # star regions (xi != 1), not only the supersonic branches
+
+
+@pytest.mark.parametrize("ndim,nf", [(1, 1), (1, 2), (2, 2), (3, 2), (3, 3)])
+@pytest.mark.parametrize("nudge", [+1.0, -1.0])
+def test_hllc_in_the_contact_frame_only_pressure_crosses_the_face(ndim, nf, nudge):
+    """(ii), with the frame shifted so that s_* = +delta (K = L) or -delta (K = R), delta = 1e-9 c: mass, energy and
+    tangential-momentum fluxes are O(delta) -- zero at round-off of their un-cancelled scales -- and the normal-momentum
+    flux is p* = p_L + rho_L (s_L - u_L)(s_* - u_L).  Holds the energy and tangential components of q*_K (nothing else
+    does where s_* != u_K), and, the two nudges giving the same flux, reading B13's "continuous across the switch"."""
+    prob, _ = wl.random_state(ndim, (4, 4, 4), nf, seed=1)
+    orc = oracle.Oracle(prob)
+    rng = np.random.default_rng(57 + 10 * ndim + nf)
+    D = ndim
+    done = 0
+    for _ in range(200):
+        wL, iL, wR, iR = _subsonic_pair(prob, rng)
+        for direction in range(ndim):
+            s_star, p_star, sL, sR = _contact_speed_and_pressure(prob, direction, wL, iL, wR, iR)
+            if not (sL < s_star < sR):
+                continue
+            cmax, rmax = max(iL["c"], iR["c"]), max(iL["rho"], iR["rho"])
+            delta = 1e-9 * cmax
+            aL, aR = wL.copy(), wR.copy()
+            aL[nf + direction] -= s_star - nudge * delta          # Galilean shift: the contact now moves at nudge * delta
+            aR[nf + direction] -= s_star - nudge * delta
+            F, uf = orc.hllc(direction, aL, aR)
+            # compression behind the outer waves (mass jump: rho*_K (s_K - s_*) = rho_K (s_K - u_K)) sets the size of q*
+            xi = max((sL - wL[nf + direction]) / (sL - s_star), (sR - wR[nf + direction]) / (sR - s_star), 1.0)
+            vt = max(np.abs(wL[nf:nf + D]).max(), np.abs(wR[nf:nf + D]).max()) + cmax
+            e_scale = rmax * (cmax ** 2 + vt ** 2) + abs(p_star)                     # rho E + p, un-cancelled
+            carried = 10.0 * xi * delta                                               # |s_*| times the compression
+            eps = 1e-13 * xi * cmax                                                   # round-off of F_K + s_K (q* - q_K)
+            assert np.all(np.abs(F[:nf]) <= (carried + eps) * rmax), F[:nf]           # mass
+            assert abs(F[nf + D]) <= (carried + eps) * e_scale, F[nf + D]             # energy
+            for t in range(D):
+                if t != direction:
+                    assert abs(F[nf + t]) <= (carried + eps) * rmax * vt, F[nf + t]   # tangential momentum
+            assert abs(F[nf + direction] - p_star) <= 1e-12 * (abs(p_star) + rmax * cmax ** 2), (F[nf + direction], p_star)
+            assert np.all(np.abs(F[nf + D + 1:]) <= carried + eps)                   # alpha rows
+            # the face velocity is the mass flux per unit upwind density (reading B12): xi_K s_*
+            xi_K = (sL - wL[nf + direction]) / (sL - s_star) if nudge > 0 else (sR - wR[nf + direction]) / (sR - s_star)
+            assert abs(uf - xi_K * nudge * delta) <= 1e-3 * xi_K * delta, (uf, xi_K * nudge * delta)
+            done += 1
+    assert done > 150
+
+
+# ---------------------------------------------------------------------------------------------
 # A7 RHS invariants                                                              pins C1, C6, C8, C9
 # ---------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("ndim,nf,periodic", [(1, 2, False), (2, 2, True), (3, 2, False), (3, 3, True)])
