@@ -50,7 +50,9 @@ typedef enum {
                               spacing with weno_order != 5 or with a non-positive ideal weight */
     MFC_ECUDA = -3,        /* CUDA runtime error (sticky); no device */
     MFC_ENOMEM = -4,       /* device or host allocation failed */
-    MFC_ENONFINITE = -5    /* mfc_advance_host: the CFL time step of the current state is NaN, infinite or zero */
+    MFC_ENONFINITE = -5,   /* mfc_advance_host: the CFL time step of the current state is NaN, infinite or zero */
+    MFC_ELIMIT = -6        /* mfc_cfl_dt_static: the grid has more interior cells than MFC_STATIC_MAX_CELLS, the most the
+                              library's fixed workspace serves; use a context (mfc_init + mfc_cfl_dt) for such a grid */
 } mfc_status;
 
 /* Cartesian grid, PAPER.md:105-124 (Eq. 6-9).  Uniform by default: dx_d = (hi_d - lo_d) / n_d.
@@ -143,6 +145,32 @@ int mfc_stage_array(mfc_ctx *ctx, int k, double **array_dev);
  * host double.  A cell whose signal speed is not finite (NaN input, negative c^2, zero density) makes the result NaN:
  * the reduction keeps NaN, it does not drop it; the call still returns MFC_OK. */
 int mfc_cfl_dt(mfc_ctx *ctx, const double *q_dev, double *dt_host, void *stream);
+
+/* The same time step for callers that cannot allocate device memory -- no context, no cudaMalloc, no synchronisation.
+ * Meant for: code that runs inside an application whose own memory pool already owns the device (a further cudaMalloc
+ * fails or eats into what the application budgeted), time loops with other streams in flight (cudaMalloc / cudaFree
+ * stall the whole device), and plug-ins that are given buffers and a stream and may only enqueue work.  Such callers
+ * cannot call mfc_init, which allocates the stage arrays and the reduction workspace.
+ *   grid, n_fluids, eos: as for mfc_init (host pointers, read during the call); uniform spacing only (edges_host must be
+ *     NULL: MFC_EUNSUPPORTED otherwise).  cfl <= 0 selects 0.3.  device < 0 selects the current device.
+ *   q_dev: the state, layout above, on `device`; only interior cells are read.  dt_dev: ONE double on `device`, written by
+ *     the kernel on `stream`; the call does not wait for it (NaN propagates as for mfc_cfl_dt).  Both belong to the caller.
+ * Workspace: one partial maximum per block of MFC_STATIC_CELLS_PER_BLOCK cells plus a counter, in a fixed
+ *   `static __device__` array of MFC_STATIC_SCRATCH_BYTES that every device holding the library keeps until the process
+ *   exits.  A grid with more than MFC_STATIC_MAX_CELLS interior cells is refused with MFC_ELIMIT before anything is
+ *   launched (256^3 and 320^3 fit, 384^3 does not).
+ * First call on a device: looks up the array's device address (cudaGetSymbolAddress); make it before any stream capture
+ *   begins.  Later calls enqueue one 8-byte memset (the counter starts every launch at zero) and one kernel.
+ * Sharing: every call on a device uses the same array, which keeps the previous call's contents.  Calls whose kernels
+ *   could run at the same time on one device (different streams without an event between them, or several host threads
+ *   doing so) race on it and return garbage; calls ordered on the GPU are safe, from any thread.
+ * Returns the same bits as mfc_cfl_dt for the same grid, fluids, cfl and state. */
+#define MFC_STATIC_CELLS_PER_BLOCK 4096
+#define MFC_STATIC_MAX_BLOCKS 8192
+#define MFC_STATIC_MAX_CELLS (MFC_STATIC_CELLS_PER_BLOCK * MFC_STATIC_MAX_BLOCKS) /* 33 554 432 */
+#define MFC_STATIC_SCRATCH_BYTES (8 * (32 + MFC_STATIC_MAX_BLOCKS))               /* 65 792 */
+int mfc_cfl_dt_static(const mfc_grid *grid, int n_fluids, const mfc_fluid *eos, double cfl, int device,
+                      const double *q_dev, double *dt_dev, void *stream);
 
 /* Whole path from HOST memory: copies q_host to the device, takes nsteps RK3 steps (each with
  * dt = dt_fixed if dt_fixed > 0, else the CFL step of the current state), copies the state back into

@@ -14,7 +14,8 @@ _HERE = Path(__file__).resolve().parent
 LIB_PATH = _HERE / "libmfc_b200.so"
 
 MFC_NG = 3
-MFC_OK, MFC_EINVAL, MFC_EUNSUPPORTED, MFC_ECUDA, MFC_ENOMEM, MFC_ENONFINITE = 0, -1, -2, -3, -4, -5
+MFC_OK, MFC_EINVAL, MFC_EUNSUPPORTED, MFC_ECUDA, MFC_ENOMEM, MFC_ENONFINITE, MFC_ELIMIT = 0, -1, -2, -3, -4, -5, -6
+MFC_STATIC_MAX_CELLS = 4096 * 8192   # mfc_cfl_dt_static: most interior cells its fixed workspace serves
 MFC_BC_PERIODIC, MFC_BC_EXTRAP, MFC_BC_HALO = 0, 1, 2
 MFC_K_RHS, MFC_K_CFL, MFC_K_PRIM, MFC_K_GHOST, MFC_K_COUNT = 0, 1, 2, 3, 4
 KERNEL_NAMES = {MFC_K_RHS: "rhs_fused", MFC_K_CFL: "cfl", MFC_K_PRIM: "prim", MFC_K_GHOST: "ghost_fill"}
@@ -23,7 +24,7 @@ MFC_STAGING_AUTO, MFC_STAGING_TMA, MFC_STAGING_CPASYNC, MFC_STAGING_ROLES = 0, 1
 # every symbol include/mfc.h declares
 EXPORTS = [
     "mfc_init", "mfc_destroy", "mfc_layout", "mfc_rhs", "mfc_rk3_step", "mfc_rk3_stage", "mfc_stage_array", "mfc_cfl_dt",
-    "mfc_advance_host",
+    "mfc_advance_host", "mfc_cfl_dt_static",
     "mfc_cons_to_prim", "mfc_line_fluxes", "mfc_profile_enable", "mfc_profile_get", "mfc_launch_count",
     "mfc_probe_dfma", "mfc_strerror", "mfc_version", "mfc_cuda_error",
 ]
@@ -81,6 +82,8 @@ def lib():
     L.mfc_rhs.argtypes = [vp, vp, vp, vp]; L.mfc_rhs.restype = C.c_int
     L.mfc_rk3_step.argtypes = [vp, vp, C.c_double, vp]; L.mfc_rk3_step.restype = C.c_int
     L.mfc_cfl_dt.argtypes = [vp, vp, dp, vp]; L.mfc_cfl_dt.restype = C.c_int
+    L.mfc_cfl_dt_static.argtypes = [C.POINTER(mfc_grid), C.c_int, C.POINTER(mfc_fluid), C.c_double, C.c_int, vp, vp, vp]
+    L.mfc_cfl_dt_static.restype = C.c_int
     L.mfc_rk3_stage.argtypes = [vp, C.c_int, vp, C.c_double, vp]; L.mfc_rk3_stage.restype = C.c_int
     L.mfc_stage_array.argtypes = [vp, C.c_int, C.POINTER(vp)]; L.mfc_stage_array.restype = C.c_int
     L.mfc_advance_host.argtypes = [vp, vp, C.c_int, C.c_double, dp, vp]; L.mfc_advance_host.restype = C.c_int
@@ -188,6 +191,26 @@ def mfc_cfl_dt(ctx, q_dev: int, stream: int = 0) -> float:
     dt = C.c_double()
     _check(lib().mfc_cfl_dt(ctx, q_dev, C.byref(dt), stream), "mfc_cfl_dt")
     return dt.value
+
+
+def mfc_cfl_dt_static(grid_n, lo, hi, fluids, q_dev: int, dt_dev: int, *, cfl: float = 0.3, device: int = -1,
+                      stream: int = 0) -> None:
+    """The CFL time step without a context and without any allocation by the library, for callers that cannot let a
+    library call cudaMalloc (see include/mfc.h).  q_dev: the state; dt_dev: address of ONE device double that the kernel
+    writes on `stream` (the call does not wait).  Uniform grids of at most MFC_STATIC_MAX_CELLS interior cells."""
+    ndim = len(grid_n)
+    g = mfc_grid()
+    g.ndim = ndim
+    for d in range(3):
+        g.n[d] = int(grid_n[d]) if d < ndim else 1
+        g.lo[d] = float(lo[d]) if d < ndim else 0.0
+        g.hi[d] = float(hi[d]) if d < ndim else 1.0
+        g.edges_host[d] = None
+    fl = (mfc_fluid * max(1, len(fluids)))()
+    for i, (gam, pinf) in enumerate(fluids):
+        fl[i].gamma, fl[i].pi_inf = float(gam), float(pinf)
+    _check(lib().mfc_cfl_dt_static(C.byref(g), len(fluids), fl, float(cfl), int(device), q_dev, dt_dev, stream),
+           "mfc_cfl_dt_static")
 
 
 def mfc_advance_host(ctx, q_host: int, nsteps: int, dt_fixed: float = 0.0, stream: int = 0) -> float:

@@ -18,7 +18,7 @@ HERE = Path(__file__).resolve().parent
 CSRC = HERE / "csrc"
 OBJ = HERE / "build"
 LIB = HERE / "libmfc_b200.so"
-SOURCES = ["mfc_api.cu", "mfc_inst_d1.cu", "mfc_inst_d2.cu", "mfc_inst_d3.cu"]
+SOURCES = ["mfc_api.cu", "mfc_static.cu", "mfc_inst_d1.cu", "mfc_inst_d2.cu", "mfc_inst_d3.cu"]
 HEADERS = [CSRC / "mfc_math.cuh", CSRC / "mfc_kernels.cuh", CSRC / "mfc_fused.cuh", CSRC / "mfc_fused_tma.cuh", CSRC / "mfc_fused_roles.cuh", CSRC / "mfc_launch.h", CSRC / "mfc_inst.cuh", HERE.parent / "include" / "mfc.h"]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "--fmad=true"]

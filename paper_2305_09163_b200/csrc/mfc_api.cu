@@ -411,6 +411,7 @@ const char *mfc_strerror(int code)
         case MFC_ECUDA: return "CUDA runtime error";
         case MFC_ENOMEM: return "out of memory";
         case MFC_ENONFINITE: return "the state is not admissible: the CFL time step is not finite";
+        case MFC_ELIMIT: return "grid too large for the fixed workspace of mfc_cfl_dt_static (MFC_STATIC_MAX_CELLS interior cells)";
     }
     return "unknown error";
 }
