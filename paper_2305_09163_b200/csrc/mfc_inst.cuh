@@ -1,5 +1,6 @@
 // Launchers of every kernel family for one value of D (= MFC_D, set by the including translation unit), all
 // NF in {1,2,3}.  One translation unit per D keeps the sm_100a compile parallel.
+#include <atomic>
 #include "mfc_kernels.cuh"
 #include "mfc_fused.cuh"
 #include "mfc_fused_tma.cuh"
@@ -76,13 +77,25 @@ static int fused_segment(const Geo &g, long long tiles, int wanted, double fill 
     return best_seg;
 }
 
-// The opt-in to more than 48 KB of dynamic shared memory is a property of the kernel, not of the launch: set once per
-// instantiation and process (a function-local static of launch_fused<D, NF, ORDER>), and its status kept: a failed
-// opt-in is reported by every later launch
+// The opt-in to more than 48 KB of dynamic shared memory is a property of the kernel ON ONE DEVICE (the function handle
+// belongs to the primary context of the device that is current): set once per instantiation and device (a function-local
+// table of launch_fused<D, NF, ORDER>, indexed by the current device; mfc_opts.device allows contexts on several GPUs in
+// one process), and its status kept: a failed opt-in is reported by every later launch on that device.  Device ordinals
+// past the table set the attribute on every launch (microseconds).
+constexpr int MFC_OPTIN_DEVICES = 64;
 #define MFC_OPTIN_SHARED(kernel, bytes)                                                                               \
     [&]() -> cudaError_t {                                                                                            \
-        static const cudaError_t st_ = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes); \
-        return st_;                                                                                                   \
+        static std::atomic<int> st_[MFC_OPTIN_DEVICES];   /* 0: not set yet; else 1 + cudaError_t of the opt-in */    \
+        int dev_ = -1;                                                                                                \
+        if (cudaGetDevice(&dev_) != cudaSuccess) return cudaErrorInvalidDevice;                                       \
+        const bool cached_ = dev_ >= 0 && dev_ < MFC_OPTIN_DEVICES;                                                   \
+        if (cached_) {                                                                                                \
+            const int v_ = st_[dev_].load(std::memory_order_acquire);                                                 \
+            if (v_) return (cudaError_t)(v_ - 1);                                                                     \
+        }                                                                                                             \
+        const cudaError_t e_ = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);      \
+        if (cached_) st_[dev_].store(1 + (int)e_, std::memory_order_release);                                         \
+        return e_;                                                                                                    \
     }()
 
 // rank-4 tensor map (x, y, z, equation) of the padded state array with a box of bx x by cells of one plane, all equations

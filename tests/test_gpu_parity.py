@@ -840,3 +840,20 @@ def test_long_run_stays_finite_and_is_bitwise_reproducible():
             outs.append(qd.cpu().numpy()[prob.interior()])
     assert np.all(np.isfinite(outs[0]))
     assert np.array_equal(outs[0], outs[1])
+
+
+# ---------------------------------------------------------------------------------------------
+# contexts on several devices of one process (mfc_opts.device): the opt-in to large dynamic shared
+# memory is per kernel AND device, so the second device's first launch must set it again
+# ---------------------------------------------------------------------------------------------
+def test_contexts_on_two_devices_in_one_process():
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two visible GPUs")
+    prob, q = wl.random_state(3, (40, 20, 12), 2, seed=9, periodic=True)
+    outs = []
+    for dev in (0, 1):
+        with torch.cuda.device(dev):
+            with Gpu(prob, device=dev) as g:
+                outs.append(g.rhs(q)[prob.interior()])
+    assert np.array_equal(outs[0], outs[1])
