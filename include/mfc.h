@@ -40,6 +40,17 @@
 extern "C" {
 #endif
 
+/* Version of this binary interface: bumped whenever a struct below changes its layout or an entry point its signature
+ * (3: mfc_grid.inv_dx, mfc_opts.abi_version, mfc_cfl_dt_static; 2: mfc_grid.edges_host, mfc_opts.staging, mfc_rhs takes a
+ * non-const q_dev and overwrites its ghost cells).  mfc_abi_version() returns the value the loaded library was built with:
+ * a caller compares it with the macro of the header it was compiled against before its first mfc_init (the Python binding
+ * does so when it loads the library), and may also store the macro in mfc_opts.abi_version to have mfc_init refuse a
+ * mismatch with MFC_EINVAL.
+ * ZERO-INITIALISE every struct of this header before setting its fields (`mfc_grid g = {0};`, memset, calloc): fields added
+ * by later versions mean "off" when zero, and mfc_init reads every field -- it dereferences edges_host[d] of each active
+ * dimension when that pointer is not NULL, so a struct built on the stack without zeroing passes it a garbage pointer. */
+#define MFC_ABI_VERSION 3
+
 #define MFC_NG 3         /* ghost layers (WENO5) */
 #define MFC_MAX_FLUIDS 3 /* compiled template set: ndim in {1,2,3} x n_fluids in {1,2,3} */
 
@@ -67,6 +78,10 @@ typedef struct {
     int n[3];        /* interior cells; entries >= ndim are ignored (treated as 1) */
     double lo[3], hi[3];
     const double *edges_host[3]; /* NULL: uniform in that dimension */
+    double inv_dx[3]; /* 0: 1 / dx_d = n_d / (hi_d - lo_d).  > 0 (uniform dimensions only): the reciprocal cell width itself.
+                         For a block of a decomposed grid (MFC_BC_HALO): pass the GLOBAL n_d / (hi_d - lo_d),
+                         so that every block, and the undivided grid, divides a face flux by the identical number; the
+                         value recomputed from a block's own lo, hi can differ in the last bits from block to block */
 } mfc_grid;
 
 /* stiffened gas, PAPER.md:54-58 (Eq. 1) */
@@ -104,6 +119,8 @@ typedef struct {
                           warps only.  A forced choice fails with MFC_ECUDA where it does not apply.  The one-loop kernels
                           compute the same bits; the kernel with Z warps sums the three directions in another order (last-bit
                           differences) */
+    int abi_version;   /* 0 (not checked) or MFC_ABI_VERSION of the header the caller was compiled against: mfc_init returns
+                          MFC_EINVAL when it differs from the library's */
 } mfc_opts;
 
 typedef struct mfc_ctx mfc_ctx;
@@ -220,6 +237,8 @@ const char *mfc_strerror(int code);
 /* Text of the CUDA runtime error behind the last MFC_ECUDA / MFC_ENOMEM a kernel launch of this context returned. */
 const char *mfc_cuda_error(const mfc_ctx *ctx);
 const char *mfc_version(void);
+/* MFC_ABI_VERSION of the loaded library (see the top of this header). */
+int mfc_abi_version(void);
 
 #ifdef __cplusplus
 }

@@ -14,6 +14,7 @@ _HERE = Path(__file__).resolve().parent
 LIB_PATH = _HERE / "libmfc_b200.so"
 
 MFC_NG = 3
+MFC_ABI_VERSION = 3   # of include/mfc.h as this binding marshals it; checked against the library when it is loaded
 MFC_OK, MFC_EINVAL, MFC_EUNSUPPORTED, MFC_ECUDA, MFC_ENOMEM, MFC_ENONFINITE, MFC_ELIMIT = 0, -1, -2, -3, -4, -5, -6
 MFC_STATIC_MAX_CELLS = 4096 * 8192   # mfc_cfl_dt_static: most interior cells its fixed workspace serves
 MFC_BC_PERIODIC, MFC_BC_EXTRAP, MFC_BC_HALO = 0, 1, 2
@@ -26,7 +27,7 @@ EXPORTS = [
     "mfc_init", "mfc_destroy", "mfc_layout", "mfc_rhs", "mfc_rk3_step", "mfc_rk3_stage", "mfc_stage_array", "mfc_cfl_dt",
     "mfc_advance_host", "mfc_cfl_dt_static",
     "mfc_cons_to_prim", "mfc_line_fluxes", "mfc_profile_enable", "mfc_profile_get", "mfc_launch_count",
-    "mfc_probe_dfma", "mfc_strerror", "mfc_version", "mfc_cuda_error",
+    "mfc_probe_dfma", "mfc_strerror", "mfc_version", "mfc_cuda_error", "mfc_abi_version",
 ]
 
 
@@ -42,7 +43,7 @@ class MfcError(RuntimeError):
 
 class mfc_grid(C.Structure):
     _fields_ = [("ndim", C.c_int), ("n", C.c_int * 3), ("lo", C.c_double * 3), ("hi", C.c_double * 3),
-                ("edges_host", C.POINTER(C.c_double) * 3)]
+                ("edges_host", C.POINTER(C.c_double) * 3), ("inv_dx", C.c_double * 3)]
 
 
 class mfc_fluid(C.Structure):
@@ -55,7 +56,7 @@ class mfc_bc(C.Structure):
 
 class mfc_opts(C.Structure):
     _fields_ = [("weno_eps", C.c_double), ("cfl", C.c_double), ("device", C.c_int), ("march_segment", C.c_int),
-                ("weno_order", C.c_int), ("kapila", C.c_int), ("staging", C.c_int)]
+                ("weno_order", C.c_int), ("kapila", C.c_int), ("staging", C.c_int), ("abi_version", C.c_int)]
 
 
 _lib = None
@@ -96,6 +97,10 @@ def lib():
     L.mfc_strerror.argtypes = [C.c_int]; L.mfc_strerror.restype = C.c_char_p
     L.mfc_version.argtypes = []; L.mfc_version.restype = C.c_char_p
     L.mfc_cuda_error.argtypes = [vp]; L.mfc_cuda_error.restype = C.c_char_p
+    L.mfc_abi_version.argtypes = []; L.mfc_abi_version.restype = C.c_int
+    if L.mfc_abi_version() != MFC_ABI_VERSION:
+        raise MfcLibraryError(f"{LIB_PATH} was built with MFC_ABI_VERSION {L.mfc_abi_version()}, this binding marshals "
+                              f"version {MFC_ABI_VERSION}: rebuild with `python -m paper_2305_09163_b200.build --force`")
     _lib = L
     return L
 
@@ -114,9 +119,11 @@ def mfc_version() -> str:
 
 
 def mfc_init(grid_n, lo, hi, fluids, bc_lo, bc_hi, *, weno_eps=1e-16, cfl=0.3, device=-1, march_segment=0, weno_order=5,
-             kapila=False, staging=MFC_STAGING_AUTO, edges=None):
+             kapila=False, staging=MFC_STAGING_AUTO, edges=None, inv_dx=None):
     """grid_n / lo / hi: one entry per active dimension; fluids: [(gamma, pi_inf), ...]; edges: per dimension the
-    n + 1 cell edges (any sequence of floats) or None for uniform spacing; returns the context handle."""
+    n + 1 cell edges (any sequence of floats) or None for uniform spacing; inv_dx: per dimension the reciprocal cell width
+    to use instead of n / (hi - lo) (blocks of a decomposed grid pass the global one), 0 or None for the default;
+    returns the context handle."""
     ndim = len(grid_n)
     g = mfc_grid()
     g.ndim = ndim
@@ -127,6 +134,7 @@ def mfc_init(grid_n, lo, hi, fluids, bc_lo, bc_hi, *, weno_eps=1e-16, cfl=0.3, d
         g.hi[d] = float(hi[d]) if d < ndim else 1.0
         b.lo[d] = int(bc_lo[d]) if d < ndim else MFC_BC_EXTRAP
         b.hi[d] = int(bc_hi[d]) if d < ndim else MFC_BC_EXTRAP
+        g.inv_dx[d] = float(inv_dx[d]) if inv_dx is not None and d < ndim and d < len(inv_dx) and inv_dx[d] else 0.0
     keep = []                                    # host edge arrays, alive until mfc_init has copied them
     for d in range(3):
         e = edges[d] if edges is not None and d < ndim and d < len(edges) else None
@@ -140,7 +148,7 @@ def mfc_init(grid_n, lo, hi, fluids, bc_lo, bc_hi, *, weno_eps=1e-16, cfl=0.3, d
     for i, (gam, pinf) in enumerate(fluids):
         fl[i].gamma, fl[i].pi_inf = float(gam), float(pinf)
     o = mfc_opts(float(weno_eps), float(cfl), int(device), int(march_segment), int(weno_order), 1 if kapila else 0,
-                 int(staging))
+                 int(staging), MFC_ABI_VERSION)
     h = C.c_void_p()
     _check(lib().mfc_init(C.byref(h), C.byref(g), len(fluids), fl, C.byref(b), C.byref(o)), "mfc_init")
     return h
@@ -206,6 +214,7 @@ def mfc_cfl_dt_static(grid_n, lo, hi, fluids, q_dev: int, dt_dev: int, *, cfl: f
         g.lo[d] = float(lo[d]) if d < ndim else 0.0
         g.hi[d] = float(hi[d]) if d < ndim else 1.0
         g.edges_host[d] = None
+        g.inv_dx[d] = 0.0
     fl = (mfc_fluid * max(1, len(fluids)))()
     for i, (gam, pinf) in enumerate(fluids):
         fl[i].gamma, fl[i].pi_inf = float(gam), float(pinf)
@@ -256,4 +265,5 @@ def init_from_problem(prob, **kw):
     D = prob.ndim
     return mfc_init(prob.n[:D], prob.lo[:D], prob.hi[:D], prob.fluids, prob.bc_lo[:D], prob.bc_hi[:D],
                     weno_eps=prob.weno_eps, cfl=prob.cfl, weno_order=getattr(prob, "weno_order", 5),
-                    kapila=getattr(prob, "kapila", False), edges=getattr(prob, "edges", None), **kw)
+                    kapila=getattr(prob, "kapila", False), edges=getattr(prob, "edges", None),
+                    inv_dx=getattr(prob, "inv_dx", None), **kw)

@@ -94,6 +94,7 @@ __global__ void __launch_bounds__(256) ghost_fill_kernel(Geo g, int neq, double 
     const int sk = bc_source(k - g.g[2], g.n[2], g.bc_lo[2], g.bc_hi[2]) + g.g[2];
     const long long dst = (long long)k * g.sz + (long long)j * g.sy + i;
     const long long src = (long long)sk * g.sz + (long long)sj * g.sy + si;
+    if (src == dst) return;     // a ghost cell of a HALO side in every dimension it is a ghost of: the caller's, left alone
     for (int e = 0; e < neq; ++e) q[(long long)e * g.cells + dst] = q[(long long)e * g.cells + src];
 }
 
@@ -268,16 +269,16 @@ int rk3(mfc_ctx *c, double *q, double dt, cudaStream_t s)
 
 int cfl_dt(mfc_ctx *c, const double *q, double *dt_host, cudaStream_t s)
 {
-    if (cudaMemsetAsync(c->min_dev, 0, sizeof(unsigned long long), s) != cudaSuccess) return MFC_ECUDA;   // max of speeds / dx
-    cudaError_t err;
+    cudaError_t err = cudaMemsetAsync(c->min_dev, 0, sizeof(unsigned long long), s);   // max of speeds / dx
+    if (err != cudaSuccess) return cuda_to_status(err, c);
     {
         Timed t(c, MFC_K_CFL, s);
         err = launch_cfl(c->ndim, c->nf, c->g, c->e, q, c->min_dev, s);
     }
-    if (err != cudaSuccess) return cuda_to_status(err);
-    if (cudaMemcpyAsync(c->min_host, c->min_dev, sizeof(unsigned long long), cudaMemcpyDeviceToHost, s) != cudaSuccess)
-        return MFC_ECUDA;
-    if (cudaStreamSynchronize(s) != cudaSuccess) return MFC_ECUDA;
+    if (err != cudaSuccess) return cuda_to_status(err, c);
+    err = cudaMemcpyAsync(c->min_host, c->min_dev, sizeof(unsigned long long), cudaMemcpyDeviceToHost, s);
+    if (err == cudaSuccess) err = cudaStreamSynchronize(s);
+    if (err != cudaSuccess) return cuda_to_status(err, c);
     double v;
     std::memcpy(&v, c->min_host, sizeof(double));
     *dt_host = c->cfl * (1.0 / v);   // v = max over cells and directions of (|u_d| + c) / dx_d
@@ -416,7 +417,9 @@ const char *mfc_strerror(int code)
     return "unknown error";
 }
 
-const char *mfc_version(void) { return "mfc-b200 0.2 (sm_100a)"; }
+const char *mfc_version(void) { return "mfc-b200 0.3 (sm_100a)"; }
+
+int mfc_abi_version(void) { return MFC_ABI_VERSION; }
 
 const char *mfc_cuda_error(const mfc_ctx *c) { return c ? cudaGetErrorString(c->last_cuda) : "no context"; }
 
@@ -424,6 +427,7 @@ int mfc_init(mfc_ctx **out, const mfc_grid *grid, int n_fluids, const mfc_fluid 
 {
     if (!out || !grid || !eos || !bc) return MFC_EINVAL;
     *out = nullptr;
+    if (opts && opts->abi_version != 0 && opts->abi_version != MFC_ABI_VERSION) return MFC_EINVAL;   // header / library mismatch
     if (grid->ndim < 1 || grid->ndim > 3 || n_fluids < 1) return MFC_EINVAL;
     if (n_fluids > MFC_MAX_FLUIDS) return MFC_EUNSUPPORTED;
     if (opts && opts->kapila && n_fluids != 2) return MFC_EUNSUPPORTED;
@@ -440,6 +444,7 @@ int mfc_init(mfc_ctx **out, const mfc_grid *grid, int n_fluids, const mfc_fluid 
             for (int i = 0; i < grid->n[d]; ++i)
                 if (!(grid->edges_host[d][i + 1] > grid->edges_host[d][i]) || !std::isfinite(grid->edges_host[d][i + 1] - grid->edges_host[d][i])) return MFC_EINVAL;
         } else if (!(grid->hi[d] > grid->lo[d])) return MFC_EINVAL;
+        if (grid->inv_dx[d] != 0.0 && (grid->edges_host[d] || !(grid->inv_dx[d] > 0.0) || !std::isfinite(grid->inv_dx[d]))) return MFC_EINVAL;
         if (bc->lo[d] < MFC_BC_PERIODIC || bc->lo[d] > MFC_BC_HALO) return MFC_EINVAL;
         if (bc->hi[d] < MFC_BC_PERIODIC || bc->hi[d] > MFC_BC_HALO) return MFC_EINVAL;
         if ((bc->lo[d] == MFC_BC_PERIODIC) != (bc->hi[d] == MFC_BC_PERIODIC)) return MFC_EINVAL;
@@ -471,7 +476,7 @@ int mfc_init(mfc_ctx **out, const mfc_grid *grid, int n_fluids, const mfc_fluid 
         g.n[d] = act ? grid->n[d] : 1;
         g.g[d] = act ? NG : 0;
         g.p[d] = g.n[d] + 2 * g.g[d];
-        g.inv_dx[d] = act && !grid->edges_host[d] ? (double)grid->n[d] / (grid->hi[d] - grid->lo[d]) : 1.0;
+        g.inv_dx[d] = act && !grid->edges_host[d] ? (grid->inv_dx[d] > 0.0 ? grid->inv_dx[d] : (double)grid->n[d] / (grid->hi[d] - grid->lo[d])) : 1.0;
         g.bc_lo[d] = act ? bc->lo[d] : MFC_BC_EXTRAP;
         g.bc_hi[d] = act ? bc->hi[d] : MFC_BC_EXTRAP;
     }
@@ -626,10 +631,11 @@ int mfc_advance_host(mfc_ctx *c, double *q_host, int nsteps, double dt_fixed, do
         cudaError_t err = cudaMalloc((void **)&c->q_own, bytes);
         if (err != cudaSuccess) {
             cudaGetLastError();
-            return cuda_to_status(err);
+            return cuda_to_status(err, c);
         }
     }
-    if (cudaMemcpyAsync(c->q_own, q_host, bytes, cudaMemcpyHostToDevice, s) != cudaSuccess) return MFC_ECUDA;
+    cudaError_t cerr = cudaMemcpyAsync(c->q_own, q_host, bytes, cudaMemcpyHostToDevice, s);
+    if (cerr != cudaSuccess) return cuda_to_status(cerr, c);
     double t = 0.0;
     for (int it = 0; it < nsteps; ++it) {
         double dt = dt_fixed;
@@ -642,8 +648,9 @@ int mfc_advance_host(mfc_ctx *c, double *q_host, int nsteps, double dt_fixed, do
         if (st) return st;
         t += dt;
     }
-    if (cudaMemcpyAsync(q_host, c->q_own, bytes, cudaMemcpyDeviceToHost, s) != cudaSuccess) return MFC_ECUDA;
-    if (cudaStreamSynchronize(s) != cudaSuccess) return MFC_ECUDA;
+    cerr = cudaMemcpyAsync(q_host, c->q_own, bytes, cudaMemcpyDeviceToHost, s);
+    if (cerr == cudaSuccess) cerr = cudaStreamSynchronize(s);
+    if (cerr != cudaSuccess) return cuda_to_status(cerr, c);
     if (t_host) *t_host = t;
     return MFC_OK;
 }
@@ -657,7 +664,7 @@ int mfc_cons_to_prim(mfc_ctx *c, const double *q_dev, double *w_dev, void *strea
         Timed t(c, MFC_K_PRIM, (cudaStream_t)stream);
         err = launch_prim(c->ndim, c->nf, c->g, c->e, q_dev, w_dev, (cudaStream_t)stream);
     }
-    return cuda_to_status(err);
+    return cuda_to_status(err, c);
 }
 
 int mfc_line_fluxes(mfc_ctx *c, int dir, int n, const double *w_dev, double *vL_dev, double *vR_dev, double *F_dev,
@@ -665,10 +672,10 @@ int mfc_line_fluxes(mfc_ctx *c, int dir, int n, const double *w_dev, double *vL_
 {
     if (!c || !w_dev || !vL_dev || !vR_dev || !F_dev || !uface_dev || n < 1 || dir < 0 || dir >= c->ndim) return MFC_EINVAL;
     DeviceGuard guard(c->device);
-    c->launch_total += 2;
     if (c->g.nu[0] && n != c->g.n[dir]) return MFC_EINVAL;     // the tables are those of the grid's own lines
+    c->launch_total += 2;                                      // (a refused call launches nothing)
     return cuda_to_status(launch_line(c->ndim, c->nf, c->order, dir, c->e, n, w_dev, vL_dev, vR_dev, F_dev, uface_dev, c->g.nu[dir], c->g.nus[dir],
-                                      (cudaStream_t)stream));
+                                      (cudaStream_t)stream), c);
 }
 
 int mfc_profile_enable(mfc_ctx *c, int on)

@@ -169,6 +169,7 @@ extern "C" int mfc_cfl_dt_static(const mfc_grid *grid, int n_fluids, const mfc_f
         if (grid->n[d] < MFC_NG) return MFC_EINVAL;
         if (grid->edges_host[d]) return MFC_EUNSUPPORTED;                // non-uniform spacing needs tables: use a context
         if (!(grid->hi[d] > grid->lo[d]) || !std::isfinite(grid->hi[d] - grid->lo[d])) return MFC_EINVAL;
+        if (grid->inv_dx[d] != 0.0 && (!(grid->inv_dx[d] > 0.0) || !std::isfinite(grid->inv_dx[d]))) return MFC_EINVAL;
         ncell *= grid->n[d];
         if (ncell > MFC_STATIC_MAX_CELLS) return MFC_ELIMIT;             // (checked per factor: no overflow)
     }
@@ -191,7 +192,7 @@ extern "C" int mfc_cfl_dt_static(const mfc_grid *grid, int n_fluids, const mfc_f
         g.n[d] = act ? grid->n[d] : 1;
         g.g[d] = act ? NG : 0;
         g.p[d] = g.n[d] + 2 * g.g[d];
-        g.inv_dx[d] = act ? (double)grid->n[d] / (grid->hi[d] - grid->lo[d]) : 1.0;
+        g.inv_dx[d] = act ? (grid->inv_dx[d] > 0.0 ? grid->inv_dx[d] : (double)grid->n[d] / (grid->hi[d] - grid->lo[d])) : 1.0;
         g.bc_lo[d] = g.bc_hi[d] = MFC_BC_EXTRAP;                         // unused: the reduction reads interior cells only
     }
     g.sy = g.p[0];

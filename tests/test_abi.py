@@ -87,3 +87,28 @@ def test_no_cpu_fallback_without_a_device(lib):
     with pytest.raises(B.MfcError) as ei:
         B.mfc_init((16,), (0.0,), (1.0,), [(1.4, 0.0)], (1,), (1,))
     assert ei.value.code == B.MFC_ECUDA
+
+
+def test_abi_version_of_header_binding_and_library_agree(lib):
+    text = (ROOT / "include" / "mfc.h").read_text()
+    assert int(re.search(r"#define\s+MFC_ABI_VERSION\s+(\d+)", text).group(1)) == B.MFC_ABI_VERSION == lib.mfc_abi_version()
+
+
+def test_init_refuses_a_caller_compiled_against_another_abi(lib):
+    g, b = B.mfc_grid(), B.mfc_bc()
+    g.ndim, g.n[0], g.lo[0], g.hi[0] = 1, 16, 0.0, 1.0
+    b.lo[0] = b.hi[0] = B.MFC_BC_EXTRAP
+    fl = (B.mfc_fluid * 1)()
+    fl[0].gamma, fl[0].pi_inf = 1.4, 0.0
+    o = B.mfc_opts()
+    o.device, o.abi_version = -1, B.MFC_ABI_VERSION - 1
+    h = C.c_void_p()
+    assert lib.mfc_init(C.byref(h), C.byref(g), 1, fl, C.byref(b), C.byref(o)) == B.MFC_EINVAL
+    assert not h.value
+
+
+def test_init_rejects_a_bad_reciprocal_width(lib):
+    for bad in (-1.0, float("inf"), float("nan")):
+        with pytest.raises(B.MfcError) as ei:
+            B.mfc_init((16,), (0.0,), (1.0,), [(1.4, 0.0)], (1,), (1,), inv_dx=(bad,))
+        assert ei.value.code == B.MFC_EINVAL
