@@ -86,24 +86,52 @@ def slab(q, d: int, side: int, ghost: bool, n_d: int):
     return q.narrow(ax, start, NG)
 
 
+def _interior_extent(q, d: int) -> int:
+    return q.shape[_axis(q.dim(), d)] - 2 * NG
+
+
+def fill_side_locally(q, d: int, side: int, nb: Optional[int], rank: int) -> bool:
+    """The two kinds of ghost slab that need no other block -- shared by the P2P exchange and the in-process one.  Returns
+    False when the slab belongs to another block (the caller then moves the neighbour's layers into it)."""
+    n_d = _interior_extent(q, d)
+    dst = slab(q, d, side, True, n_d)
+    if nb is None:                                           # physical boundary, zero-gradient (PAPER.md:168 as read in B14)
+        ax = _axis(q.dim(), d)
+        edge = q.narrow(ax, NG if side == 0 else NG + n_d - 1, 1)
+        dst.copy_(edge.expand_as(dst))
+        return True
+    if nb == rank:                                           # the block is its own periodic neighbour: local wrap
+        dst.copy_(slab(q, d, 1 - side, False, n_d))
+        return True
+    return False
+
+
+def fill_ghosts_in_process(blocks, ndim: int, decomp: Decomposition) -> None:
+    """The same fill for ALL blocks of a decomposition held by one process (``blocks[rank]``, tensors on one device): the
+    slab a rank would receive is copied straight out of the neighbour's array.  Same slabs, same order (dimension by
+    dimension over the full padded extent of the others, every block finishing dimension d before any starts d + 1) as
+    ``fill_ghosts``; only the wire is missing.  Used to check a decomposed run against the undivided one on a single GPU."""
+    for d in range(ndim):
+        for rank, q in enumerate(blocks):
+            for side in (0, 1):
+                nb = decomp.neighbour(rank, d, side)
+                if not fill_side_locally(q, d, side, nb, rank):
+                    src = blocks[nb]
+                    slab(q, d, side, True, _interior_extent(q, d)).copy_(slab(src, d, 1 - side, False, _interior_extent(src, d)))
+
+
 def fill_ghosts(q, ndim: int, decomp: Decomposition, rank: int, group=None) -> None:
     """Fills every ghost cell of the block ``q`` (torch tensor [eq, z, y, x], CPU or CUDA) in place."""
     import torch
     import torch.distributed as dist
 
     for d in range(ndim):
-        n_d = q.shape[_axis(q.dim(), d)] - 2 * NG
+        n_d = _interior_extent(q, d)
         sends, recvs, landing = [], [], []
         for side in (0, 1):
             nb = decomp.neighbour(rank, d, side)
             dst = slab(q, d, side, True, n_d)
-            if nb is None:                                   # physical boundary, zero-gradient (PAPER.md:168 as read in B14)
-                ax = _axis(q.dim(), d)
-                edge = q.narrow(ax, NG if side == 0 else NG + n_d - 1, 1)
-                dst.copy_(edge.expand_as(dst))
-            elif nb == rank:                                 # the block is its own periodic neighbour: local wrap
-                dst.copy_(slab(q, d, 1 - side, False, n_d))
-            else:
+            if not fill_side_locally(q, d, side, nb, rank):
                 # what I send through face `side` are my interior layers next to it; what lands in my ghost layers of that
                 # side are the neighbour's layers next to ITS opposite face.  The tag names the sender's face (gloo matches
                 # by tag); NCCL matches the operations between two ranks in posting order, so when one rank is the
@@ -192,8 +220,11 @@ def split_problem(prob, q_global, decomp: Decomposition, rank: int):
         else:
             h = prob.dx[d]
             lo[d], hi[d] = prob.lo[d] + rng[d][0] * h, prob.lo[d] + rng[d][1] * h
+    # the reciprocal width every block divides by is the GLOBAL n / (hi - lo), formed as mfc_init forms it (ADVICE r2:
+    # recomputed from a block's own lo, hi it differs in the last bits from block to block)
+    inv_dx = tuple(float(prob.n[d]) / (prob.hi[d] - prob.lo[d]) if d < prob.ndim and edges[d] is None else 0.0 for d in range(3))
     local = dataclasses.replace(prob, name=f"{prob.name}_r{rank}", n=n, lo=tuple(lo), hi=tuple(hi),
-                                edges=tuple(edges) if any(e is not None for e in edges) else None)
+                                edges=tuple(edges) if any(e is not None for e in edges) else None, inv_dx=inv_dx)
     ql = np.zeros(local.shape())
     it = prob.interior()
     sl = [slice(None)]
@@ -204,3 +235,76 @@ def split_problem(prob, q_global, decomp: Decomposition, rank: int):
             sl.append(slice(0, 1))
     ql[local.interior()] = q_global[tuple(sl)]
     return local, ql
+
+
+class LocalBlocks:
+    """Every block of a decomposition in ONE process on the current device: one context per block, the in-process ghost
+    fill between them, the global CFL minimum.  A decomposed run without the wire -- what a single GPU can check of
+    PAPER.md:176-182: partitioning, slab geometry, the order of exchange and stages, the per-stage entry points."""
+
+    def __init__(self, prob, q_global, decomp: Decomposition, **kw):
+        import dataclasses
+
+        import torch
+
+        from . import binding as B
+
+        self.B, self.torch, self.prob, self.decomp = B, torch, prob, decomp
+        halo = (BC_HALO,) * 3
+        self.local, self.ctx, self.q, self.stage = [], [], [], []
+        for rank in range(decomp.world):
+            lp, ql = split_problem(prob, q_global, decomp, rank)
+            ctx = B.init_from_problem(dataclasses.replace(lp, bc_lo=halo, bc_hi=halo), **kw)
+            self.local.append(lp)
+            self.ctx.append(ctx)
+            self.q.append(torch.from_numpy(ql).cuda())
+            self.stage.append([None] + [torch.as_tensor(_DevArray(B.mfc_stage_array(ctx, k), lp.shape()), device="cuda") for k in (1, 2)])
+
+    def close(self):
+        for ctx in self.ctx:
+            self.B.mfc_destroy(ctx)
+        self.ctx = []
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    @property
+    def _stream(self) -> int:
+        return self.torch.cuda.current_stream().cuda_stream
+
+    def cfl_dt(self) -> float:
+        return min(self.B.mfc_cfl_dt(ctx, q.data_ptr(), self._stream) for ctx, q in zip(self.ctx, self.q))
+
+    def rhs(self):
+        """-> one array per block: L of the decomposed state (ghost entries unspecified)"""
+        fill_ghosts_in_process(self.q, self.prob.ndim, self.decomp)
+        outs = [self.torch.full_like(q, float("nan")) for q in self.q]
+        for ctx, q, o in zip(self.ctx, self.q, outs):
+            self.B.mfc_rhs(ctx, q.data_ptr(), o.data_ptr(), self._stream)
+        return outs
+
+    def rk3_step(self, dt: float) -> None:
+        for k in range(3):
+            arrays = self.q if k == 0 else [st[k] for st in self.stage]
+            fill_ghosts_in_process(arrays, self.prob.ndim, self.decomp)
+            for ctx, q in zip(self.ctx, self.q):
+                self.B.mfc_rk3_stage(ctx, k, q.data_ptr(), dt, self._stream)
+
+    def gather(self, blocks=None):
+        """Stitches the interiors of ``blocks`` (default: the state) into a global padded numpy array (ghost cells zero)."""
+        import numpy as np
+
+        blocks = self.q if blocks is None else blocks
+        self.torch.cuda.synchronize()
+        out = np.zeros(self.prob.shape())
+        it = self.prob.interior()
+        for rank, (lp, b) in enumerate(zip(self.local, blocks)):
+            rng = self.decomp.local_cells(rank, self.prob.n)
+            sl = [slice(None)]
+            for ax, d in ((1, 2), (2, 1), (3, 0)):
+                sl.append(slice(it[ax].start + rng[d][0], it[ax].start + rng[d][1]) if d < self.prob.ndim else slice(0, 1))
+            out[tuple(sl)] = b.cpu().numpy()[lp.interior()]
+        return out

@@ -56,6 +56,9 @@ class Problem:
     kapila: bool = False  # K div(u) source of PAPER.md Eq. 2 on the alpha row (two fluids); False = Allaire
     # non-uniform Cartesian spacing: per dimension the n + 1 edges of the interior cells, or None (uniform)
     edges: Tuple | None = None
+    # per dimension the reciprocal cell width to hand to mfc_init instead of n / (hi - lo) (mfc_grid.inv_dx): set on the
+    # blocks of a decomposed grid to the global value, so that every block divides by the identical number
+    inv_dx: Tuple | None = None
 
     @property
     def nf(self) -> int:

@@ -121,3 +121,45 @@ def test_single_block_fill_is_the_plain_ghost_fill():
     t = torch.from_numpy(q.copy())
     halo.fill_ghosts(t, 3, dec, 0)
     assert np.array_equal(t.numpy(), ref)
+
+
+# ---------------------------------------------------------------------------------------------
+# the in-process fill (all blocks of a decomposition in one process: what the one-GPU decomposition tests use) moves the
+# same slabs as the P2P exchange: held to the same reference
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dims,ndim,n,periodic_dims", [
+    ((2, 1, 1), 3, (9, 7, 8), (0, 1, 2)),
+    ((2, 1, 1), 3, (9, 7, 8), ()),
+    ((1, 2, 2), 3, (8, 9, 11), (0, 2)),
+    ((2, 2, 2), 3, (10, 9, 11), (1,)),
+    ((3, 2, 1), 2, (13, 9), (0,)),
+    ((4, 1, 1), 1, (23,), (0,)),
+])
+def test_in_process_fill_matches_numpy_pad_of_the_global_array(dims, ndim, n, periodic_dims):
+    import torch
+    prob, q, ref = _global_case(ndim, n, periodic_dims)
+    dec = halo.Decomposition(dims, prob.bc_lo, prob.bc_hi)
+    blocks, locals_ = [], []
+    for rank in range(dec.world):
+        local, ql = halo.split_problem(prob, q, dec, rank)
+        core = ql[local.interior()].copy()
+        ql[...] = np.random.default_rng(100 + rank).normal(size=ql.shape)      # garbage in the ghosts
+        ql[local.interior()] = core
+        blocks.append(torch.from_numpy(ql))
+        locals_.append(local)
+    halo.fill_ghosts_in_process(blocks, ndim, dec)
+    for rank, (local, t) in enumerate(zip(locals_, blocks)):
+        cells = dec.local_cells(rank, prob.n)
+        sl = [slice(None)]
+        for ax, d in ((1, 2), (2, 1), (3, 0)):
+            sl.append(slice(cells[d][0], cells[d][1] + 2 * NG) if d < ndim else slice(0, 1))
+        assert np.array_equal(t.numpy(), ref[tuple(sl)]), rank
+
+
+def test_blocks_of_a_split_problem_carry_the_global_reciprocal_width():
+    prob, q, _ = _global_case(3, (10, 9, 11), ())
+    dec = halo.Decomposition((2, 2, 2), prob.bc_lo, prob.bc_hi)
+    want = tuple(float(prob.n[d]) / (prob.hi[d] - prob.lo[d]) for d in range(3))
+    for rank in range(dec.world):
+        local, _ = halo.split_problem(prob, q, dec, rank)
+        assert local.inv_dx == want
