@@ -186,12 +186,13 @@ def time_workload(B, torch, prob, q, local, steps, warmup, segment=0):
         B.mfc_destroy(ctx)
 
 
-def extra_config_line(B, torch, name, prob, q, local, steps, fp64_tf, hbm_peak):
+def extra_config_line(B, torch, name, prob, q, local, steps, fp64_tf, hbm_peak, note=None):
     """One entry of `extra_configs`: the same step, event-timed, on a non-headline workload, with its roofline fractions."""
     ms_step, prof, ok = time_workload(B, torch, prob, q, local, steps, 3)
     flops_cell, bytes_cell = rhs_algorithmic(prob)
     t_avg = prof["rhs_fused"]["ms_avg"] * 1e-3
     return {"workload": f"{prob.name} {prob.n[0]}x{prob.n[1]}x{prob.n[2]} nf={prob.nf} neq={prob.neq} ({name})", "steps": steps,
+            **({"note": note} if note else {}),
             "ms_per_step": ms_step, "value": ms_step * 1e6 / (prob.cells * prob.neq * RHS_PER_STEP), "unit": UNIT,
             "cells_steps_per_s": prob.cells / (ms_step * 1e-3),
             "kernels_ms_avg": {k: v["ms_avg"] for k, v in prof.items() if v["launches"]},
@@ -348,10 +349,16 @@ def run_ours(args):
             # regime (cfg2), the three-fluid 384^3 case (cfg4) and the headline data on the Eq. 15 stretched grid
             from paper_2305_09163_b200 import workloads as wl
             extra = []
-            for name, make in (("BASELINE.json configs[2]", lambda: wl.cfg2()), ("BASELINE.json configs[4]", lambda: wl.cfg4()),
-                               ("configs[3] on the Eq. 15 stretched grid", lambda: (lambda pq: (wl.with_stretched_grid(pq[0]), pq[1]))(wl.cfg3()))):
+            small = ("the 1D / 2D kernel (rhs_fused_plane_kernel) at the parity-test size: the state fits L2 and a step is a "
+                     "handful of microsecond launches plus the host round trip of mfc_cfl_dt -- launch- and latency-bound, "
+                     "not a roofline figure")
+            for name, make, nsteps, note in (
+                    ("BASELINE.json configs[0], 1D shock tube", lambda: wl.cfg0(), 50, small),
+                    ("BASELINE.json configs[1], 2D advected interface", lambda: wl.cfg1(), 50, small),
+                    ("BASELINE.json configs[2]", lambda: wl.cfg2(), 5, None), ("BASELINE.json configs[4]", lambda: wl.cfg4(), 5, None),
+                    ("configs[3] on the Eq. 15 stretched grid", lambda: (lambda pq: (wl.with_stretched_grid(pq[0]), pq[1]))(wl.cfg3()), 5, None)):
                 p2, q2 = make()
-                extra.append(extra_config_line(B, torch, name, p2, q2, local, 5, fp64_tf, hbm_peak))
+                extra.append(extra_config_line(B, torch, name, p2, q2, local, nsteps, fp64_tf, hbm_peak, note))
                 del q2
                 torch.cuda.empty_cache()
             out["extra_configs"] = extra
@@ -398,13 +405,15 @@ def cpu_baseline(args):
     sec = sum(times) / len(times)
     oracle.set_threads(1)
     try:
-        n1 = max(32, n_sample // 2)
+        n1 = args.cpu_n1
         prob1, times1, _ = oracle_step_time(args, n1, 1, 0)
     finally:
         oracle.set_threads(cores)
     sec1 = times1[0]
+    full = {"cfg0": 1000, "cfg1": 512, "cfg2": 128, "cfg3": 256, "cfg4": 384}[args.workload]   # default sizes of workloads.py
+    size = f"at its full size, {n_sample}^3 cells" if n_sample == full else f"shrunk to {n_sample}^3 cells"
     return {"value": sec * 1e9 / (prob.cells * prob.neq * RHS_PER_STEP), "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": f"{prob.name} shrunk to {n_sample}^3 cells, 2 steps of (CFL + RK3) with the OpenMP oracle, {sec:.2f} s/step",
+            "sample": f"{prob.name} {size}, 2 steps of (CFL + RK3) with the OpenMP oracle, {sec:.2f} s/step",
             "cpu_model": cpu_model(),
             "one_thread": {"value": sec1 * 1e9 / (prob1.cells * prob1.neq * RHS_PER_STEP), "unit": UNIT, "cores": 1,
                            "sample": f"{prob1.name} shrunk to {n1}^3 cells, 1 step of (CFL + RK3), {sec1:.2f} s/step"}}
@@ -440,7 +449,8 @@ def main():
     ap.add_argument("--n", type=int, default=None, help="override cells per dimension (default: the config's size)")
     ap.add_argument("--segment", type=int, default=0, help="z planes each block of the fused kernel marches (0 = heuristic)")
     ap.add_argument("--e2e-steps", type=int, default=5)
-    ap.add_argument("--cpu-n", type=int, default=128, help="cells per dimension of the cpu_baseline sample")
+    ap.add_argument("--cpu-n", type=int, default=256, help="cells per dimension of the all-cores cpu_baseline sample (256 = the headline workload at full size: about 4 s per step on 16 cores)")
+    ap.add_argument("--cpu-n1", type=int, default=64, help="cells per dimension of the one-thread cpu_baseline sample")
     ap.add_argument("--ref-n", type=int, default=96, help="cells per dimension of the --impl reference sample")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-extra", action="store_true", help="skip the extra_configs leg (cfg2, cfg4, stretched cfg3)")

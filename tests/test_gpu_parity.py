@@ -516,8 +516,13 @@ def subbox_reference(prob, q_full, lo, b):
     D = prob.ndim
     idx = [np.arange(lo[d] - wl.NG, lo[d] + b + wl.NG) % prob.n[d] + wl.NG for d in range(D)]   # wrap: periodic cut-outs
     cut = q_full[np.ix_(np.arange(prob.neq), idx[2], idx[1], idx[0])]
+    edges = None
+    if prob.edges is not None:
+        # stretched grid: the cut-out keeps its own cell edges (boxes must then stay clear of the boundaries: no wrap)
+        assert all(lo[d] >= wl.NG and lo[d] + b + wl.NG <= prob.n[d] for d in range(D))
+        edges = tuple(np.asarray(prob.edges[d])[lo[d] - wl.NG:lo[d] + b + wl.NG + 1].copy() for d in range(D))
     sub = wl.Problem("sub", D, (b + 6,) * 3, (0.0,) * 3, tuple((b + 6) * prob.dx[d] for d in range(3)), prob.fluids,
-                     (wl.BC_EXTRAP,) * 3, (wl.BC_EXTRAP,) * 3, weno_eps=prob.weno_eps)
+                     (wl.BC_EXTRAP,) * 3, (wl.BC_EXTRAP,) * 3, weno_eps=prob.weno_eps, edges=edges)
     qs = np.zeros(sub.shape())
     qs[sub.interior()] = cut
     L = oracle.Oracle(sub).rhs(qs)
@@ -561,6 +566,17 @@ def test_rhs_full_size_cfg4_sampled():
     rng = np.random.default_rng(1)
     boxes = [tuple(int(v) for v in rng.integers(0, 384, size=3)) for _ in range(10)]
     boxes += [(0, 0, 0), (379, 379, 379), (380, 5, 190)]                      # wrap around the periodic faces
+    check_full_size_sampled(prob, q, boxes)
+
+
+def test_rhs_full_size_cfg3_stretched_sampled():
+    """The benchmarked stretched configuration (bench.py extra_configs: cfg3 on the Eq. 15 grid, 256^3, default launch
+    configuration) against the oracle on sampled boxes, the strongly stretched region and the finest cells included."""
+    prob, q = wl.cfg3()
+    prob = wl.with_stretched_grid(prob)
+    rng = np.random.default_rng(5)
+    boxes = [tuple(int(v) for v in rng.integers(3, 256 - 13, size=3)) for _ in range(10)]
+    boxes += [(3, 3, 3), (243, 243, 243), (123, 123, 123), (3, 123, 243)]
     check_full_size_sampled(prob, q, boxes)
 
 
@@ -622,6 +638,22 @@ def test_rk3_parity_cfg3_reduced():
 
 def test_rk3_parity_cfg4_reduced():
     prob, q = wl.cfg4(n=64)
+    check_rk(prob, q)
+
+
+def test_rk3_parity_cfg4_half_size():
+    """cfg4 at 192^3 (three fluids; 16 x 16 tiles x several z segments, the launch shape of the 384^3 the bench times, not
+    the two tile rows of the 64^3 case above) for the 10 steps north_star names.  192^3 rather than 384^3: the oracle
+    needs about 2.5 s per step here against 20 s and 21 GB of host memory at full size."""
+    prob, q = wl.cfg4(n=192)
+    check_rk(prob, q)
+
+
+def test_rhs_and_rk3_parity_kapila_on_a_stretched_grid():
+    import dataclasses
+    prob, q = wl.random_state(3, (40, 29, 33), 2, seed=92, periodic=False)
+    prob = dataclasses.replace(wl.with_stretched_grid(prob), kapila=True)
+    check_rhs(prob, q)
     check_rk(prob, q)
 
 
