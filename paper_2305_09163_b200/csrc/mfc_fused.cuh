@@ -106,6 +106,15 @@ struct NoHook {
 struct NuPlane {
     const double *tx, *ty;
     int sx, sy;
+    __device__ __forceinline__ NuRef x(int col) const { return NuRef{tx + col, sx}; }
+    __device__ __forceinline__ NuRef y(int row) const { return NuRef{ty + row, sy}; }
+};
+// the same for a block that has staged its columns -1 .. FTX and rows -1 .. TY in shared memory (rows of S doubles)
+template <int S>
+struct NuPlaneShared {
+    const double *tx, *ty;
+    __device__ __forceinline__ NuShared<S> x(int col) const { return NuShared<S>{tx + col}; }
+    __device__ __forceinline__ NuShared<S> y(int row) const { return NuShared<S>{ty + row}; }
 };
 
 // `early` runs at the top of the first FP64-heavy block and `mid` at the top of the second: the caller's loads,
@@ -128,8 +137,8 @@ __device__ __forceinline__ void inplane_sync()
 // dealt round-robin to ALL threads (two rounds in 3D with two fluids, the second one leaving out the two warps that
 // solve the rim faces), so that no warp reaches the barrier much later than the others.  A right state is the
 // left state of the mirrored stencil: one code path, the side only flips the sign of the stride. ----
-template <int D, int NF, int TY, int ORDER, bool NU>
-__device__ __forceinline__ void rim_units(const InplaneBufs<D, NF, TY> &B, const Eos &eos, const NuPlane &nup)
+template <int D, int NF, int TY, int ORDER, bool NU, class NP>
+__device__ __forceinline__ void rim_units(const InplaneBufs<D, NF, TY> &B, const Eos &eos, const NP &nup)
 {
     using C = FusedCfg<D, NF, TY>;
     constexpr int NEQ = C::NEQ, NT = C::NT, PPL = C::PPL, HY = C::HY;
@@ -144,7 +153,7 @@ __device__ __forceinline__ void rim_units(const InplaneBufs<D, NF, TY> &B, const
                 int e, r, st;
                 const double *pb;
                 double *dst;
-                NuRef nr{nullptr, 0};                               // (non-uniform: the rim cell's coefficients)
+                decltype(nup.x(0)) nr{};                            // (non-uniform: the rim cell's coefficients)
                 if (D >= 2 && u < UY) {
                     const int kind = u / (FTX * NEQ), rem = u - kind * (FTX * NEQ);
                     e = rem / FTX;
@@ -152,7 +161,7 @@ __device__ __forceinline__ void rim_units(const InplaneBufs<D, NF, TY> &B, const
                     pb = P + e * PPL + (kind == 0 ? HY - 1 : HY + TY) * FPX + NG + r;
                     st = kind == 0 ? FPX : -FPX;
                     dst = (kind == 0 ? B.HyL : B.HyR) + e * FTX + r;
-                    if constexpr (NU) nr = NuRef{nup.ty + (kind == 0 ? -1 : TY), nup.sy};
+                    if constexpr (NU) nr = nup.y(kind == 0 ? -1 : TY);
                 } else {
                     const int v = u - UY, kind = v / (TY * NEQ), rem = v - kind * (TY * NEQ);
                     e = rem / TY;
@@ -160,7 +169,7 @@ __device__ __forceinline__ void rim_units(const InplaneBufs<D, NF, TY> &B, const
                     pb = P + e * PPL + (r + HY) * FPX + NG + (kind == 0 ? -1 : (kind == 1 ? FTX : 0));
                     st = kind == 0 ? 1 : -1;
                     dst = (kind == 0 ? B.HxL : (kind == 1 ? B.HxR : B.ExR)) + e * TY + r;
-                    if constexpr (NU) nr = NuRef{nup.tx + (kind == 0 ? -1 : (kind == 1 ? FTX : 0)), nup.sx};
+                    if constexpr (NU) nr = nup.x(kind == 0 ? -1 : (kind == 1 ? FTX : 0));
                 }
                 double v, other;
                 if constexpr (NU) {                                 // the coefficients are not mirror images: both sides, one kept
@@ -207,10 +216,11 @@ __device__ __forceinline__ void rim_face_x(const InplaneBufs<D, NF, TY> &B, cons
 }
 
 // XP: variables whose x reconstruction runs before barrier S1
-template <int D, int NF, int TY, int ORDER, bool NU = false, int GT = 0, int XP = MFC_XPRE, class Early = NoHook, class Mid = NoHook>
+template <int D, int NF, int TY, int ORDER, bool NU = false, int GT = 0, int XP = MFC_XPRE, class Early = NoHook, class Mid = NoHook,
+          class NP = NuPlane>
 __device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, const Eos &eos, double cx, double cy,
                                            double (&acc)[2 * NF + D], Early early = Early(), Mid mid = Mid(),
-                                           const NuPlane &nup = NuPlane{nullptr, nullptr, 0, 0})
+                                           const NP &nup = NP{})
 {
     using C = FusedCfg<D, NF, TY>;
     using I = Idx<D, NF>;
@@ -234,7 +244,7 @@ __device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, cons
         for (int e = 0; e < NEQ; ++e) {
             const double *s5 = pc + e * PPL;
             reconstruct<ORDER, NU>(s5[0], s5[-FPX] - s5[-2 * FPX], s5[0] - s5[-FPX], s5[FPX] - s5[0], s5[2 * FPX] - s5[FPX], eos.weno_eps4, vLy[e], vRy[e],
-                                   NuRef{nup.ty + j, nup.sy});
+                                   nup.y(j));
         }
 #pragma unroll
         for (int e = 0; e < NEQ; ++e) B.X[e * NT + tid] = vRy[e];
@@ -246,7 +256,7 @@ __device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, cons
 #pragma unroll
     for (int e = 0; e < XPRE; ++e) {
         const double *s5 = pc + e * PPL;
-        reconstruct<ORDER, NU>(s5[0], s5[-1] - s5[-2], s5[0] - s5[-1], s5[1] - s5[0], s5[2] - s5[1], eos.weno_eps4, vL[e], vR[e], NuRef{nup.tx + i, nup.sx});
+        reconstruct<ORDER, NU>(s5[0], s5[-1] - s5[-2], s5[0] - s5[-1], s5[1] - s5[0], s5[2] - s5[1], eos.weno_eps4, vL[e], vR[e], nup.x(i));
     }
     inplane_sync<GT>();                                             // S1: rim states and y right states are visible
 
@@ -257,7 +267,7 @@ __device__ __forceinline__ void inplane_xy(const InplaneBufs<D, NF, TY> &B, cons
 #pragma unroll
         for (int e = XPRE; e < NEQ; ++e) {
             const double *s5 = pc + e * PPL;
-            reconstruct<ORDER, NU>(s5[0], s5[-1] - s5[-2], s5[0] - s5[-1], s5[1] - s5[0], s5[2] - s5[1], eos.weno_eps4, vL[e], vR[e], NuRef{nup.tx + i, nup.sx});
+            reconstruct<ORDER, NU>(s5[0], s5[-1] - s5[-2], s5[0] - s5[-1], s5[1] - s5[0], s5[2] - s5[1], eos.weno_eps4, vL[e], vR[e], nup.x(i));
         }
 #pragma unroll
         for (int e = 0; e < NEQ; ++e) {

@@ -15,7 +15,7 @@
 // (A finer split -- X, Y, Z, rim and conversion warps with five loops -- is in the history of this file: parity-exact but
 // bound by instruction fetch: 85 KB of loop code per multiprocessor against a 32 KB instruction cache.)
 #pragma once
-#include <cstdio>
+#include <type_traits>
 #include "mfc_fused_tma.cuh"
 
 #ifndef MFC_ROLES_XPRE
@@ -51,22 +51,7 @@ __device__ __forceinline__ void mbar_wait_sleep(unsigned long long *bar, unsigne
         "}\n" ::"r"(smem_addr(bar)), "r"(parity)
         : "memory");
 }
-#ifdef MFC_ROLES_DEBUG
-static __device__ __noinline__ void mbar_wait_dbg(unsigned long long *bar, unsigned parity, int line)
-{
-    for (long long it = 0; it < (1ll << 24); ++it) {
-        unsigned ok;
-        asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}\n" : "=r"(ok) : "r"(smem_addr(bar)), "r"(parity) : "memory");
-        if (ok) return;
-    }
-    if ((threadIdx.x & 31) == 0) printf("STUCK block %d warp %d line %d parity %u\n", blockIdx.x, threadIdx.x >> 5, line, parity);
-    __nanosleep(1000000);
-    asm volatile("trap;");
-}
-#define RWAIT(bar, parity) mbar_wait_dbg(bar, parity, __LINE__)
-#else
 #define RWAIT(bar, parity) mbar_wait_sleep(bar, parity)
-#endif
 __device__ __forceinline__ void group_barrier(int id, int threads) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory"); }
 __device__ __forceinline__ void fence_async_proxy() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
@@ -102,6 +87,15 @@ struct RolesCfg {
     enum { FULL_P = 0, PRIM_P = 2, FULL_LZ = 4, EMPTY_LZ = 6, FULL_SQ = 8, NBAR = FULL_SQ + TY, TMEM_WORD = NBAR, NWORDS = NBAR + 1 };
     static constexpr int doubles = oBar + r16(NWORDS);
     static constexpr int bytes = doubles * (int)sizeof(double);
+    // non-uniform spacing only (after everything else): the block's slice of the coefficient tables, coefficient-major in rows
+    // of NUS doubles -- columns -1 .. FTX of the x table, rows -1 .. TY of the y table -- and, per Z warp, the coefficients
+    // of the one cell along z its lanes are reconstructing
+    static constexpr int NUS = FTX + 2;
+    static constexpr int oNuX = doubles, oNuY = oNuX + NU_NC * NUS, oNuZ = oNuY + NU_NC * NUS;
+    static constexpr int bytes_nu = (oNuZ + 4 * 32) * (int)sizeof(double);
+    static_assert(TY + 2 <= NUS, "y rows fit a row of the slice");
+    // (three fluids: the slices do not fit beside the tile; that instantiation keeps reading the tables from global memory)
+    static constexpr bool nu_staged = bytes_nu <= 227 * 1024;
     static constexpr unsigned plane_bytes = NEQ * PPL * sizeof(double);
     static constexpr unsigned row_bytes = NEQ * CW * sizeof(double);
     // tensor memory of a Z thread, per row: ring of four primitive planes, parked left state, previous flux + face
@@ -150,6 +144,16 @@ __global__ void __launch_bounds__(RolesCfg<NF, TY>::THREADS, 1)
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         fence_async_proxy();
     }
+    constexpr bool NUSM = NU && R::nu_staged;                       // coefficient tables staged in shared memory
+    if constexpr (NUSM) {
+        // the tile's columns and rows do not change along the march: their coefficients come from global memory once
+        // (rows of the tables are padded past the last cell, mfc_api.cu nu_tables: ragged tiles read defined entries)
+        for (int t = tid; t < NU_NC * R::NUS; t += R::THREADS) {
+            const int k = t / R::NUS, c = t - k * R::NUS;
+            sm[R::oNuX + t] = __ldg(g.nu[0] + x0 + NG - 1 + c + k * g.nus[0]);
+            sm[R::oNuY + t] = c < TY + 2 ? __ldg(g.nu[1] + y0 + NG - 1 + c + k * g.nus[1]) : 0.0;
+        }
+    }
     if (warp == 0) tmem_alloc512(tmem_word);
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
@@ -189,8 +193,13 @@ __global__ void __launch_bounds__(RolesCfg<NF, TY>::THREADS, 1)
             asm volatile("" : "+d"(coef));
             double cx = coef * g.inv_dx[0], cy = coef * g.inv_dx[1], czp = cz;
             if constexpr (NU) {                                     // the cell's own widths (Eq. 8-9): entry 27 of the tables
-                cx = coef * __ldg(g.nu[0] + x0 + NG + i + 27 * g.nus[0]);
-                cy = coef * __ldg(g.nu[1] + y0 + NG + j + 27 * g.nus[1]);
+                if constexpr (NUSM) {
+                    cx = coef * sm[R::oNuX + 27 * R::NUS + 1 + i];
+                    cy = coef * sm[R::oNuY + 27 * R::NUS + 1 + j];
+                } else {
+                    cx = coef * __ldg(g.nu[0] + x0 + NG + i + 27 * g.nus[0]);
+                    cy = coef * __ldg(g.nu[1] + y0 + NG + j + 27 * g.nus[1]);
+                }
                 czp = coef * __ldg(g.nu[2] + k0 + u + NG + 27 * g.nus[2]);
             }
             RWAIT(bars + R::PRIM_P + b, par(u >> 1));                  // the Z warps have made plane u primitives (own cells and halo)
@@ -203,7 +212,10 @@ __global__ void __launch_bounds__(RolesCfg<NF, TY>::THREADS, 1)
                     for (int e = 0; e < NEQ; ++e) prefetch_l2(o.qn + (long long)e * g.cells + cell + g.sz);
                 }
             };
-            if constexpr (NU) {                                     // per-index coefficient tables of the tile's columns and rows
+            if constexpr (NUSM) {                                   // per-index coefficient tables of the tile's columns and rows
+                inplane_xy<D, NF, TY, ORDER, true, NT, MFC_ROLES_XPRE>(b ? B1 : B0, eos, cx, cy, acc, early, NoHook(),
+                                                                       NuPlaneShared<R::NUS>{sm + R::oNuX + 1, sm + R::oNuY + 1});
+            } else if constexpr (NU) {
                 inplane_xy<D, NF, TY, ORDER, true, NT, MFC_ROLES_XPRE>(b ? B1 : B0, eos, cx, cy, acc, early, NoHook(),
                                                                        NuPlane{g.nu[0] + x0 + NG, g.nu[1] + y0 + NG, g.nus[0], g.nus[1]});
             } else {
@@ -254,6 +266,15 @@ __global__ void __launch_bounds__(RolesCfg<NF, TY>::THREADS, 1)
             const int v = n - 2 * NG + 1;                           // plane m - 2: reconstructed along z; own cells -> staged plane
             double *const Lz = sm + R::oLz + lzb(u) * R::nL;
             if (u >= R::NLZ) RWAIT(bars + R::EMPTY_LZ + lzb(u), par(lzk(u - R::NLZ)));
+            if constexpr (NUSM) {
+                // the coefficients of cell m - 2 = k0 + v along z are the same for every thread and row: one load per lane,
+                // then read back by all lanes (the warp's own 32 doubles of shared memory)
+                if (n >= 4) {
+                    __syncwarp();
+                    if (lane < NU_NC) sm[R::oNuZ + 32 * zw + lane] = __ldg(g.nu[2] + k0 + v + NG + lane * g.nus[2]);
+                    __syncwarp();
+                }
+            }
 #pragma unroll 1
             for (int r = 0; r < R::ZR; ++r) {
                 const int row = R::ZR * zw + r;
@@ -276,8 +297,12 @@ __global__ void __launch_bounds__(RolesCfg<NF, TY>::THREADS, 1)
                     // window of the variables 2p, 2p + 1: planes m - 4 .. m - 1 from the ring (plane m - 4 sits in the slot
                     // plane m is about to take); reconstruct cell m - 2
                     double vLn[TV], vR[NEQ], vbE = 0.0, vbA[I::NA > 0 ? I::NA : 1];
-                    NuRef nz{nullptr, 0};
-                    if constexpr (NU) nz = NuRef{g.nu[2] + k0 + v + NG, g.nus[2]};     // tables of cell m - 2 = k0 + v
+                    // tables of cell m - 2 = k0 + v (NU only)
+                    const typename std::conditional<NUSM, NuShared<1>, NuRef>::type nz = [&]() {
+                        if constexpr (NUSM) return NuShared<1>{sm + R::oNuZ + 32 * zw};
+                        else if constexpr (NU) return NuRef{g.nu[2] + k0 + v + NG, g.nus[2]};
+                        else return NuRef{nullptr, 0};
+                    }();
 #pragma unroll
                     for (int p = 0; p < (NEQ + 1) / 2; ++p) {
                         unsigned w4[4], w3[4], w2[4], w1[4];

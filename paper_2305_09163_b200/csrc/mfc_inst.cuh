@@ -152,8 +152,9 @@ static cudaError_t launch_fused_nu(const typename GeoOf<NU>::type &g, const Eos 
                 const int rseg = fused_segment(g, (long long)ntx * rnty, segment, 1.0);
                 const unsigned rblocks = (unsigned)((long long)ntx * rnty * ((g.n[2] + rseg - 1) / rseg));
                 if (encode_state_map(&tm_plane, g, C::NEQ, q, FPX, RTY + 2 * NG) && encode_state_map(&tm_col, g, C::NEQ, q, R::CW, 1)) {
-                    if ((st = MFC_OPTIN_SHARED((rhs_fused_roles_kernel<NF, RTY, ORDER, NU>), R::bytes)) != cudaSuccess) return st;
-                    rhs_fused_roles_kernel<NF, RTY, ORDER, NU><<<rblocks, R::THREADS, R::bytes, s>>>(tm_plane, tm_col, g, e, o, ntx, rnty, rseg);
+                    constexpr int rbytes = NU && R::nu_staged ? R::bytes_nu : R::bytes;
+                    if ((st = MFC_OPTIN_SHARED((rhs_fused_roles_kernel<NF, RTY, ORDER, NU>), rbytes)) != cudaSuccess) return st;
+                    rhs_fused_roles_kernel<NF, RTY, ORDER, NU><<<rblocks, R::THREADS, rbytes, s>>>(tm_plane, tm_col, g, e, o, ntx, rnty, rseg);
                     return cudaSuccess;
                 }
             }
