@@ -109,12 +109,12 @@ struct NuPlane {
     __device__ __forceinline__ NuRef x(int col) const { return NuRef{tx + col, sx}; }
     __device__ __forceinline__ NuRef y(int row) const { return NuRef{ty + row, sy}; }
 };
-// the same for a block that has staged its columns -1 .. FTX and rows -1 .. TY in shared memory (rows of S doubles)
-template <int S>
+// the same for a block that has staged the records (NuRec, mfc_math.cuh) of its columns -1 .. FTX and rows -1 .. TY in
+// shared memory: shared-space addresses of the records of column 0 and row 0
 struct NuPlaneShared {
-    const double *tx, *ty;
-    __device__ __forceinline__ NuShared<S> x(int col) const { return NuShared<S>{tx + col}; }
-    __device__ __forceinline__ NuShared<S> y(int row) const { return NuShared<S>{ty + row}; }
+    unsigned ax, ay;
+    __device__ __forceinline__ NuRec x(int col) const { return NuRec{ax + (unsigned)(col * NU_REC * 8)}; }
+    __device__ __forceinline__ NuRec y(int row) const { return NuRec{ay + (unsigned)(row * NU_REC * 8)}; }
 };
 
 // `early` runs at the top of the first FP64-heavy block and `mid` at the top of the second: the caller's loads,

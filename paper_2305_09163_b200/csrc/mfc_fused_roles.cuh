@@ -87,13 +87,12 @@ struct RolesCfg {
     enum { FULL_P = 0, PRIM_P = 2, FULL_LZ = 4, EMPTY_LZ = 6, FULL_SQ = 8, NBAR = FULL_SQ + TY, TMEM_WORD = NBAR, NWORDS = NBAR + 1 };
     static constexpr int doubles = oBar + r16(NWORDS);
     static constexpr int bytes = doubles * (int)sizeof(double);
-    // non-uniform spacing only (after everything else): the block's slice of the coefficient tables, coefficient-major in rows
-    // of NUS doubles -- columns -1 .. FTX of the x table, rows -1 .. TY of the y table -- and, per Z warp, the coefficients
-    // of the one cell along z its lanes are reconstructing
-    static constexpr int NUS = FTX + 2;
-    static constexpr int oNuX = doubles, oNuY = oNuX + NU_NC * NUS, oNuZ = oNuY + NU_NC * NUS;
-    static constexpr int bytes_nu = (oNuZ + 4 * 32) * (int)sizeof(double);
-    static_assert(TY + 2 <= NUS, "y rows fit a row of the slice");
+    // non-uniform spacing only (after everything else): the block's slice of the coefficient tables as one record of NU_REC
+    // doubles per cell (NuRec, mfc_math.cuh) -- columns -1 .. FTX of the x table, rows -1 .. TY of the y table -- and, per Z
+    // warp, the record of the one cell along z its lanes are reconstructing
+    static constexpr int oNuX = doubles, oNuY = oNuX + (FTX + 2) * NU_REC, oNuZ = oNuY + (TY + 2) * NU_REC;
+    static constexpr int bytes_nu = (oNuZ + 4 * NU_REC) * (int)sizeof(double);
+    static_assert(NU_REC % 2 == 0 && doubles % 2 == 0, "records are read with 16-byte loads");
     // (three fluids: the slices do not fit beside the tile; that instantiation keeps reading the tables from global memory)
     static constexpr bool nu_staged = bytes_nu <= 227 * 1024;
     static constexpr unsigned plane_bytes = NEQ * PPL * sizeof(double);
@@ -148,10 +147,10 @@ __global__ void __launch_bounds__(RolesCfg<NF, TY>::THREADS, 1)
     if constexpr (NUSM) {
         // the tile's columns and rows do not change along the march: their coefficients come from global memory once
         // (rows of the tables are padded past the last cell, mfc_api.cu nu_tables: ragged tiles read defined entries)
-        for (int t = tid; t < NU_NC * R::NUS; t += R::THREADS) {
-            const int k = t / R::NUS, c = t - k * R::NUS;
-            sm[R::oNuX + t] = __ldg(g.nu[0] + x0 + NG - 1 + c + k * g.nus[0]);
-            sm[R::oNuY + t] = c < TY + 2 ? __ldg(g.nu[1] + y0 + NG - 1 + c + k * g.nus[1]) : 0.0;
+        for (int t = tid; t < NU_NC * (FTX + 2 + TY + 2); t += R::THREADS) {
+            const int k = t / (FTX + 2 + TY + 2), c = t - k * (FTX + 2 + TY + 2);
+            if (c < FTX + 2) sm[R::oNuX + c * NU_REC + nu_rec_pos(k)] = __ldg(g.nu[0] + x0 + NG - 1 + c + k * g.nus[0]);
+            else sm[R::oNuY + (c - FTX - 2) * NU_REC + nu_rec_pos(k)] = __ldg(g.nu[1] + y0 + NG - 1 + (c - FTX - 2) + k * g.nus[1]);
         }
     }
     if (warp == 0) tmem_alloc512(tmem_word);
@@ -194,8 +193,8 @@ __global__ void __launch_bounds__(RolesCfg<NF, TY>::THREADS, 1)
             double cx = coef * g.inv_dx[0], cy = coef * g.inv_dx[1], czp = cz;
             if constexpr (NU) {                                     // the cell's own widths (Eq. 8-9): entry 27 of the tables
                 if constexpr (NUSM) {
-                    cx = coef * sm[R::oNuX + 27 * R::NUS + 1 + i];
-                    cy = coef * sm[R::oNuY + 27 * R::NUS + 1 + j];
+                    cx = coef * sm[R::oNuX + (1 + i) * NU_REC + nu_rec_pos(27)];
+                    cy = coef * sm[R::oNuY + (1 + j) * NU_REC + nu_rec_pos(27)];
                 } else {
                     cx = coef * __ldg(g.nu[0] + x0 + NG + i + 27 * g.nus[0]);
                     cy = coef * __ldg(g.nu[1] + y0 + NG + j + 27 * g.nus[1]);
@@ -214,7 +213,7 @@ __global__ void __launch_bounds__(RolesCfg<NF, TY>::THREADS, 1)
             };
             if constexpr (NUSM) {                                   // per-index coefficient tables of the tile's columns and rows
                 inplane_xy<D, NF, TY, ORDER, true, NT, MFC_ROLES_XPRE>(b ? B1 : B0, eos, cx, cy, acc, early, NoHook(),
-                                                                       NuPlaneShared<R::NUS>{sm + R::oNuX + 1, sm + R::oNuY + 1});
+                                                                       NuPlaneShared{smem_addr(sm + R::oNuX + NU_REC), smem_addr(sm + R::oNuY + NU_REC)});
             } else if constexpr (NU) {
                 inplane_xy<D, NF, TY, ORDER, true, NT, MFC_ROLES_XPRE>(b ? B1 : B0, eos, cx, cy, acc, early, NoHook(),
                                                                        NuPlane{g.nu[0] + x0 + NG, g.nu[1] + y0 + NG, g.nus[0], g.nus[1]});
@@ -271,7 +270,7 @@ __global__ void __launch_bounds__(RolesCfg<NF, TY>::THREADS, 1)
                 // then read back by all lanes (the warp's own 32 doubles of shared memory)
                 if (n >= 4) {
                     __syncwarp();
-                    if (lane < NU_NC) sm[R::oNuZ + 32 * zw + lane] = __ldg(g.nu[2] + k0 + v + NG + lane * g.nus[2]);
+                    if (lane < NU_NC) sm[R::oNuZ + NU_REC * zw + nu_rec_pos(lane)] = __ldg(g.nu[2] + k0 + v + NG + lane * g.nus[2]);
                     __syncwarp();
                 }
             }
@@ -298,8 +297,8 @@ __global__ void __launch_bounds__(RolesCfg<NF, TY>::THREADS, 1)
                     // plane m is about to take); reconstruct cell m - 2
                     double vLn[TV], vR[NEQ], vbE = 0.0, vbA[I::NA > 0 ? I::NA : 1];
                     // tables of cell m - 2 = k0 + v (NU only)
-                    const typename std::conditional<NUSM, NuShared<1>, NuRef>::type nz = [&]() {
-                        if constexpr (NUSM) return NuShared<1>{sm + R::oNuZ + 32 * zw};
+                    const typename std::conditional<NUSM, NuRec, NuRef>::type nz = [&]() {
+                        if constexpr (NUSM) return NuRec{smem_addr(sm + R::oNuZ + NU_REC * zw)};
                         else if constexpr (NU) return NuRef{g.nu[2] + k0 + v + NG, g.nus[2]};
                         else return NuRef{nullptr, 0};
                     }();
