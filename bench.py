@@ -3,7 +3,7 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg3] [--n 256]
 
-One "step" is one pass of the whole path over the workload: the CFL reduction (mfc_cfl_dt) and one 3-stage
+One "step" is one pass of the whole path over the workload (mfc_step_cfl): the CFL reduction (mfc_cfl_dt) and one 3-stage
 TVD-RK step (mfc_rk3_step = 3 launches of the fused kernel: ghost fill + cons->prim, WENO5+HLLC in x, y, z, flux
 difference, stage combine).  The workload is BASELINE.json configs[3] (256^3 two-fluid bubble cloud), seeded and synthetic.
 N > 1 (torchrun): independent replicas, one per GPU, no data-path collective ("replicas only", DESIGN.md);
@@ -165,7 +165,7 @@ def time_workload(B, torch, prob, q, local, steps, warmup, segment=0):
         stream = torch.cuda.current_stream().cuda_stream
         qd = torch.from_numpy(q).cuda()
         for _ in range(max(3, warmup)):
-            B.mfc_rk3_step(ctx, qd.data_ptr(), B.mfc_cfl_dt(ctx, qd.data_ptr(), stream), stream)
+            B.mfc_step_cfl(ctx, qd.data_ptr(), stream)
         torch.cuda.synchronize()
         for kid in range(B.MFC_K_COUNT):
             B.mfc_profile_get(ctx, kid, reset=True)
@@ -173,7 +173,7 @@ def time_workload(B, torch, prob, q, local, steps, warmup, segment=0):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
         for _ in range(steps):
-            B.mfc_rk3_step(ctx, qd.data_ptr(), B.mfc_cfl_dt(ctx, qd.data_ptr(), stream), stream)
+            B.mfc_step_cfl(ctx, qd.data_ptr(), stream)
         e1.record()
         torch.cuda.synchronize()
         prof = {}
@@ -240,9 +240,7 @@ def run_ours(args):
     torch.cuda.synchronize()
 
     def step():
-        dt = B.mfc_cfl_dt(ctx, qd.data_ptr(), stream)
-        B.mfc_rk3_step(ctx, qd.data_ptr(), dt, stream)
-        return dt
+        return B.mfc_step_cfl(ctx, qd.data_ptr(), stream)    # CFL reduction, then the three stages at that dt
 
     for _ in range(max(3, args.warmup)):
         step()
@@ -328,7 +326,7 @@ def run_ours(args):
             "config": {"workload": f"{prob.name} {prob.n[0]}x{prob.n[1]}x{prob.n[2]} nf={prob.nf} neq={neq} (BASELINE.json configs[{args.workload[3:]}])",
                        "cells_per_gpu": prob.cells, "rhs_per_step": RHS_PER_STEP, "parallelism": f"replicas x{world}",
                        "l2": "inputs larger than L2 (each state array >= 1 GB at 256^3)", "march_segment": args.segment,
-                       "step": "mfc_cfl_dt + mfc_rk3_step"},
+                       "step": "mfc_step_cfl (= mfc_cfl_dt + mfc_rk3_step, the first ghost fill enqueued before the wait for dt)"},
             "cells_steps_per_s": prob.cells * world / (ms_step * 1e-3),
             "gpu_launches": launches,
             "kernels": prof,

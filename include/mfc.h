@@ -27,7 +27,7 @@
  *   stream or process that allocates tensor memory on the same device (any tcgen05 GEMM, e.g. a bf16 matmul) is
  *   serialised against it by the hardware allocator: it waits, results are unaffected.
  * Streams: `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  All work is
- *   enqueued on it.  Only mfc_cfl_dt, mfc_advance_host, mfc_profile_get and mfc_probe_dfma synchronise.
+ *   enqueued on it.  Only mfc_cfl_dt, mfc_step_cfl, mfc_advance_host, mfc_profile_get and mfc_probe_dfma synchronise.
  * Errors: every function returns MFC_OK (0) or a negative mfc_status; nothing is thrown or printed.
  *   A context is not thread-safe.  State admissibility is not checked on the hot path: non-finite or
  *   inadmissible states propagate as NaN.  There is no CPU fallback: without a CUDA device mfc_init fails
@@ -162,6 +162,14 @@ int mfc_stage_array(mfc_ctx *ctx, int k, double **array_dev);
  * host double.  A cell whose signal speed is not finite (NaN input, negative c^2, zero density) makes the result NaN:
  * the reduction keeps NaN, it does not drop it; the call still returns MFC_OK. */
 int mfc_cfl_dt(mfc_ctx *ctx, const double *q_dev, double *dt_host, void *stream);
+
+/* mfc_cfl_dt followed by mfc_rk3_step with that time step, as one call: q_dev advances by the CFL step of the state it
+ * holds; *dt_host (may be NULL) receives the step taken.  Same kernels, same bits as the two calls.  The host needs dt before
+ * it can launch the first stage, so the call waits once for the reduction; the ghost fill of the first stage (which does not
+ * depend on dt) is enqueued before that wait, so the device is busy during the round trip -- at 128^3 the pair of calls
+ * leaves it idle for 3 % of a step.  A time step that is NaN, infinite or not positive is not taken: MFC_ENONFINITE, the
+ * interior of q_dev untouched (its ghost cells filled), *dt_host holding the offending value. */
+int mfc_step_cfl(mfc_ctx *ctx, double *q_dev, double *dt_host, void *stream);
 
 /* The same time step for callers that cannot allocate device memory -- no context, no cudaMalloc, no synchronisation.
  * Meant for: code that runs inside an application whose own memory pool already owns the device (a further cudaMalloc

@@ -25,7 +25,7 @@ MFC_STAGING_AUTO, MFC_STAGING_TMA, MFC_STAGING_CPASYNC, MFC_STAGING_ROLES = 0, 1
 # every symbol include/mfc.h declares
 EXPORTS = [
     "mfc_init", "mfc_destroy", "mfc_layout", "mfc_rhs", "mfc_rk3_step", "mfc_rk3_stage", "mfc_stage_array", "mfc_cfl_dt",
-    "mfc_advance_host", "mfc_cfl_dt_static",
+    "mfc_advance_host", "mfc_cfl_dt_static", "mfc_step_cfl",
     "mfc_cons_to_prim", "mfc_line_fluxes", "mfc_profile_enable", "mfc_profile_get", "mfc_launch_count",
     "mfc_probe_dfma", "mfc_strerror", "mfc_version", "mfc_cuda_error", "mfc_abi_version",
 ]
@@ -85,6 +85,7 @@ def lib():
     L.mfc_cfl_dt.argtypes = [vp, vp, dp, vp]; L.mfc_cfl_dt.restype = C.c_int
     L.mfc_cfl_dt_static.argtypes = [C.POINTER(mfc_grid), C.c_int, C.POINTER(mfc_fluid), C.c_double, C.c_int, vp, vp, vp]
     L.mfc_cfl_dt_static.restype = C.c_int
+    L.mfc_step_cfl.argtypes = [vp, vp, dp, vp]; L.mfc_step_cfl.restype = C.c_int
     L.mfc_rk3_stage.argtypes = [vp, C.c_int, vp, C.c_double, vp]; L.mfc_rk3_stage.restype = C.c_int
     L.mfc_stage_array.argtypes = [vp, C.c_int, C.POINTER(vp)]; L.mfc_stage_array.restype = C.c_int
     L.mfc_advance_host.argtypes = [vp, vp, C.c_int, C.c_double, dp, vp]; L.mfc_advance_host.restype = C.c_int
@@ -198,6 +199,13 @@ def mfc_stage_array(ctx, k: int) -> int:
 def mfc_cfl_dt(ctx, q_dev: int, stream: int = 0) -> float:
     dt = C.c_double()
     _check(lib().mfc_cfl_dt(ctx, q_dev, C.byref(dt), stream), "mfc_cfl_dt")
+    return dt.value
+
+
+def mfc_step_cfl(ctx, q_dev: int, stream: int = 0) -> float:
+    """One step at the CFL time step of the current state (mfc_cfl_dt + mfc_rk3_step as one call); -> the step taken."""
+    dt = C.c_double()
+    _check_ctx(lib().mfc_step_cfl(ctx, q_dev, C.byref(dt), stream), "mfc_step_cfl", ctx)
     return dt.value
 
 

@@ -147,6 +147,7 @@ struct mfc_ctx {
     double *nu_dev[3] = {nullptr, nullptr, nullptr};   // non-uniform spacing: per-direction coefficient tables
     unsigned long long *min_dev = nullptr;
     unsigned long long *min_host = nullptr;  // pinned
+    cudaEvent_t dt_ready = nullptr;          // recorded behind the copy of the reduction's result: the host waits for it alone
     bool profile = false;
     std::vector<mfc::EventPair> pending;
     std::vector<cudaEvent_t> pool;
@@ -222,16 +223,21 @@ int cuda_to_status(cudaError_t e, mfc_ctx *c = nullptr)
 
 // One evaluation of L(q_in): the ghost cells of q_in are filled in memory (a0), then one launch computes
 // out = base + coef L(q_in), base described by `o` (SweepOut, mfc_launch.h).
-int eval_L(mfc_ctx *c, double *q_in, const SweepOut &o, cudaStream_t s)
+int fill_ghosts_of(mfc_ctx *c, double *q_in, cudaStream_t s)
 {
-    cudaError_t err = cudaSuccess;
     bool all_halo = true;
     for (int d = 0; d < c->ndim; ++d) all_halo = all_halo && c->g.bc_lo[d] == MFC_BC_HALO && c->g.bc_hi[d] == MFC_BC_HALO;
-    if (!all_halo) {
-        Timed t(c, MFC_K_GHOST, s);
-        err = launch_ghost_fill(c->g, c->neq, q_in, s);
-        if (err != cudaSuccess) return cuda_to_status(err, c);
+    if (all_halo) return MFC_OK;
+    Timed t(c, MFC_K_GHOST, s);
+    return cuda_to_status(launch_ghost_fill(c->g, c->neq, q_in, s), c);
+}
+int eval_L(mfc_ctx *c, double *q_in, const SweepOut &o, cudaStream_t s, bool ghosts_filled = false)
+{
+    if (!ghosts_filled) {
+        const int st = fill_ghosts_of(c, q_in, s);
+        if (st) return st;
     }
+    cudaError_t err = cudaSuccess;
     {
         Timed t(c, MFC_K_RHS, s);
         err = launch_rhs(c->ndim, c->nf, c->order, c->g, c->e, q_in, o, c->segment, c->staging, s);
@@ -241,13 +247,13 @@ int eval_L(mfc_ctx *c, double *q_in, const SweepOut &o, cudaStream_t s)
 
 // 3-stage TVD Runge-Kutta.  Every stage is out = ca qn + cb (qs + dt L(qs)).  A stage reads its
 // neighbours' cells of qs, so it never writes the array it evaluates L on: q -> q1 -> q2 -> q.
-int rk3_stage(mfc_ctx *c, int stage, double *q, double dt, cudaStream_t s)
+int rk3_stage(mfc_ctx *c, int stage, double *q, double dt, cudaStream_t s, bool ghosts_filled = false)
 {
     SweepOut f{};
     switch (stage) {
         case 0:   // q1 = q + dt L(q)
             f.out = c->q1; f.qs = q; f.qn = q; f.ca = 0.0; f.cb = 1.0; f.coef = dt; f.nbase = 1;
-            return eval_L(c, q, f, s);
+            return eval_L(c, q, f, s, ghosts_filled);
         case 1:   // q2 = 3/4 q + 1/4 (q1 + dt L(q1))
             f.out = c->q2; f.qs = c->q1; f.qn = q; f.ca = 0.75; f.cb = 0.25; f.coef = 0.25 * dt; f.nbase = 2;
             return eval_L(c, c->q1, f, s);
@@ -267,7 +273,8 @@ int rk3(mfc_ctx *c, double *q, double dt, cudaStream_t s)
     return MFC_OK;
 }
 
-int cfl_dt(mfc_ctx *c, const double *q, double *dt_host, cudaStream_t s)
+// the reduction and the copy of its result, enqueued; cfl_dt_finish waits for them
+int cfl_dt_enqueue(mfc_ctx *c, const double *q, cudaStream_t s)
 {
     cudaError_t err = cudaMemsetAsync(c->min_dev, 0, sizeof(unsigned long long), s);   // max of speeds / dx
     if (err != cudaSuccess) return cuda_to_status(err, c);
@@ -277,12 +284,45 @@ int cfl_dt(mfc_ctx *c, const double *q, double *dt_host, cudaStream_t s)
     }
     if (err != cudaSuccess) return cuda_to_status(err, c);
     err = cudaMemcpyAsync(c->min_host, c->min_dev, sizeof(unsigned long long), cudaMemcpyDeviceToHost, s);
-    if (err == cudaSuccess) err = cudaStreamSynchronize(s);
+    if (err == cudaSuccess) err = cudaEventRecord(c->dt_ready, s);
+    return cuda_to_status(err, c);
+}
+// waits for the copy only (not for work enqueued behind it)
+int cfl_dt_finish(mfc_ctx *c, double *dt_host)
+{
+    const cudaError_t err = cudaEventSynchronize(c->dt_ready);
     if (err != cudaSuccess) return cuda_to_status(err, c);
     double v;
     std::memcpy(&v, c->min_host, sizeof(double));
     *dt_host = c->cfl * (1.0 / v);   // v = max over cells and directions of (|u_d| + c) / dx_d
     return MFC_OK;
+}
+
+// One step at the CFL time step of the current state (a6 then a0 - a5, three times).  The host needs dt before it can launch
+// the first stage (dt is a kernel argument), so every step has one device -> host round trip; the ghost fill of stage 0
+// does not depend on dt and is enqueued BEFORE the wait, so the device works through the round trip instead of idling.
+int step_cfl(mfc_ctx *c, double *q, double *dt_out, cudaStream_t s)
+{
+    int st = cfl_dt_enqueue(c, q, s);
+    if (st) return st;
+    st = fill_ghosts_of(c, q, s);
+    if (st) return st;
+    double dt = 0.0;
+    st = cfl_dt_finish(c, &dt);
+    if (st) return st;
+    if (dt_out) *dt_out = dt;
+    if (!std::isfinite(dt) || !(dt > 0.0)) return MFC_ENONFINITE;    // inadmissible state: do not step on
+    for (int stage = 0; stage < 3; ++stage) {
+        st = rk3_stage(c, stage, q, dt, s, stage == 0);
+        if (st) return st;
+    }
+    return MFC_OK;
+}
+
+int cfl_dt(mfc_ctx *c, const double *q, double *dt_host, cudaStream_t s)
+{
+    const int st = cfl_dt_enqueue(c, q, s);
+    return st ? st : cfl_dt_finish(c, dt_host);
 }
 
 __global__ void __launch_bounds__(256) dfma_probe_kernel(double *out, int iters, double m, double a)
@@ -514,6 +554,7 @@ int mfc_init(mfc_ctx **out, const mfc_grid *grid, int n_fluids, const mfc_fluid 
     if (err == cudaSuccess) err = cudaMalloc((void **)&c->q2, bytes);
     if (err == cudaSuccess) err = cudaMalloc((void **)&c->min_dev, sizeof(unsigned long long));
     if (err == cudaSuccess) err = cudaMallocHost((void **)&c->min_host, sizeof(unsigned long long));
+    if (err == cudaSuccess) err = cudaEventCreateWithFlags(&c->dt_ready, cudaEventDisableTiming);
     if (err == cudaSuccess) {   // reciprocal seeds of gamma_i - 1, as the device computes them (mfc_math.cuh div_seed)
         double *tmp = nullptr;
         err = cudaMalloc((void **)&tmp, 2 * MAX_NF * sizeof(double));
@@ -569,6 +610,7 @@ void mfc_destroy(mfc_ctx *c)
         for (int d = 0; d < 3; ++d) cudaFree(c->nu_dev[d]);
         cudaFree(c->min_dev);
         if (c->min_host) cudaFreeHost(c->min_host);
+        if (c->dt_ready) cudaEventDestroy(c->dt_ready);
     }
     delete c;
 }
@@ -614,6 +656,13 @@ int mfc_stage_array(mfc_ctx *c, int k, double **array_dev)
     return MFC_OK;
 }
 
+int mfc_step_cfl(mfc_ctx *c, double *q_dev, double *dt_host, void *stream)
+{
+    if (!c || !q_dev) return MFC_EINVAL;
+    DeviceGuard guard(c->device);
+    return step_cfl(c, q_dev, dt_host, (cudaStream_t)stream);
+}
+
 int mfc_cfl_dt(mfc_ctx *c, const double *q_dev, double *dt_host, void *stream)
 {
     if (!c || !q_dev || !dt_host) return MFC_EINVAL;
@@ -639,13 +688,8 @@ int mfc_advance_host(mfc_ctx *c, double *q_host, int nsteps, double dt_fixed, do
     double t = 0.0;
     for (int it = 0; it < nsteps; ++it) {
         double dt = dt_fixed;
-        if (!(dt_fixed > 0.0)) {
-            const int st = cfl_dt(c, c->q_own, &dt, s);
-            if (st) return st;
-            if (!std::isfinite(dt) || !(dt > 0.0)) return MFC_ENONFINITE;    // inadmissible state: do not step on
-        }
-        const int st = rk3(c, c->q_own, dt, s);
-        if (st) return st;
+        const int st = dt_fixed > 0.0 ? rk3(c, c->q_own, dt, s) : step_cfl(c, c->q_own, &dt, s);
+        if (st) return st;                                           // (MFC_ENONFINITE: the step was not taken)
         t += dt;
     }
     cerr = cudaMemcpyAsync(q_host, c->q_own, bytes, cudaMemcpyDeviceToHost, s);

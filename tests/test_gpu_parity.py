@@ -837,6 +837,31 @@ def test_advance_host_equals_device_path():
         assert np.array_equal(qp[it], ref1[it])
 
 
+def test_step_cfl_equals_cfl_dt_followed_by_rk3_step():
+    """mfc_step_cfl only reorders the enqueue (first ghost fill before the wait for dt): same dt, same bits; an inadmissible
+    state is refused with MFC_ENONFINITE and its interior left alone."""
+    prob, q = wl.random_state(3, (40, 29, 33), 2, seed=33, periodic=False)
+    it = prob.interior()
+    with Gpu(prob) as g:
+        qa, qb = g.to_dev(q), g.to_dev(q)
+        dts_a, dts_b = [], []
+        for _ in range(4):
+            dts_a.append(B.mfc_cfl_dt(g.ctx, qa.data_ptr(), g.stream))
+            B.mfc_rk3_step(g.ctx, qa.data_ptr(), dts_a[-1], g.stream)
+            dts_b.append(B.mfc_step_cfl(g.ctx, qb.data_ptr(), g.stream))
+        g.torch.cuda.synchronize()
+        assert dts_a == dts_b
+        assert np.array_equal(qa.cpu().numpy()[it], qb.cpu().numpy()[it])
+        bad = q.copy()
+        bad[it][prob.nf + prob.ndim][3, 5, 7] = np.nan
+        qc = g.to_dev(bad)
+        with pytest.raises(B.MfcError) as ei:
+            B.mfc_step_cfl(g.ctx, qc.data_ptr(), g.stream)
+        assert ei.value.code == B.MFC_ENONFINITE
+        g.torch.cuda.synchronize()
+        assert np.array_equal(qc.cpu().numpy()[it], bad[it], equal_nan=True)
+
+
 def test_profile_hooks_count_launches_and_time():
     prob, q = wl.random_state(3, (32, 32, 32), 2, seed=1)
     with Gpu(prob) as g:
