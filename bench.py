@@ -40,12 +40,12 @@ def measured_peaks():
     return 6650.0, "fallback"
 
 
-TRAFFIC_CSV = os.path.join("profiles", "r02_dram_traffic.csv")
+TRAFFIC_CSV = os.path.join("profiles", "r03_dram_traffic.csv")
 
 
 def ncu_traffic(workload: str, kernel: str):
     """(dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` on `workload`, provenance) from the committed
-    ncu capture (profiles/r02_dram_traffic.csv: one `ncu --set full` run, its command and the commit it profiled are in
+    ncu capture (profiles/r03_dram_traffic.csv: one `ncu --set full` run, its command and the commit it profiled are in
     the file).  It is RECORDED, not measured in this run: the provenance string says which commit it belongs to.
     (None, None) when no capture is recorded for the workload."""
     path = os.path.join(ROOT, TRAFFIC_CSV)
@@ -311,12 +311,12 @@ def run_ours(args):
         else:
             roof = {"kernel": dom, "bound": "alu", "achieved": ach_tf, "peak": fp64_tf, "unit": "TFLOP/s",
                     "frac": ach_tf / fp64_tf, "traffic": traffic,
-                    "peak_source": "mfc_probe_dfma (register-resident DFMA chains), measured in this run; DESIGN.md 6.1"}
+                    "peak_source": "mfc_probe_dfma (register-resident DFMA chains, faster of two operand shapes: 99.95 % of the FP64 pipe under ncu, profiles/r03_probe.md), measured in this run; DESIGN.md 6.1"}
         roof.update({"algorithmic_flops_per_cell": flops_cell, "algorithmic_bytes_per_cell": bytes_cell,
                      "avg_launch_ms": prof[dom]["ms_avg"], "hbm_frac": ach_gbs / hbm_peak, "fp64_frac": ach_tf / fp64_tf,
                      "hbm_peak_gbs": hbm_peak, "hbm_peak_source": f"MEASURED_PEAKS.json ({hbm_src})",
                      "traffic_source": traffic_src,
-                     "fp64_pipe_busy_recorded": "profiles/r02_ncu_full.md (sm__inst_executed_pipe_fp64, executed-flop fraction)",
+                     "fp64_pipe_busy_recorded": "profiles/r03_ncu_full.md (sm__inst_executed_pipe_fp64 68 %, executed-flop fraction)",
                      "fp64_peak_measured_tflops": fp64_tf, "fp64_peak_nominal_tflops": FP64_NOMINAL_TFLOPS,
                      "kernel_ms_sum_over_step_ms": sum(v["ms_total"] for v in prof.values()) / ms_total})
         out = {
