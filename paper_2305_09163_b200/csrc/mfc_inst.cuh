@@ -112,12 +112,31 @@ static bool encode_state_map(CUtensorMap *map, const Geo &g, int neq, const doub
         return reinterpret_cast<encode_fn>(p);
     }();
     if (!fn) return false;
+    // a map depends on the array's address, the padded extents and the box only: the last few are kept per host thread (an RK
+    // step alternates between three arrays and two boxes), so a launch normally encodes nothing
+    struct Key { const double *base; int p0, p1, p2, neq, bx, by; };
+    struct Slot { Key k; CUtensorMap m; bool used; };
+    static thread_local Slot cache[8] = {};
+    static thread_local unsigned next = 0;
+    const Key key{base, g.p[0], g.p[1], g.p[2], neq, bx, by};
+    for (const Slot &sl : cache)
+        if (sl.used && sl.k.base == key.base && sl.k.p0 == key.p0 && sl.k.p1 == key.p1 && sl.k.p2 == key.p2 && sl.k.neq == key.neq &&
+            sl.k.bx == key.bx && sl.k.by == key.by) {
+            *map = sl.m;
+            return true;
+        }
     const cuuint64_t dims[4] = {(cuuint64_t)g.p[0], (cuuint64_t)g.p[1], (cuuint64_t)g.p[2], (cuuint64_t)neq};
     const cuuint64_t strides[3] = {(cuuint64_t)g.sy * 8, (cuuint64_t)g.sz * 8, (cuuint64_t)g.cells * 8};
     const cuuint32_t box[4] = {(cuuint32_t)bx, (cuuint32_t)by, 1, (cuuint32_t)neq};
     const cuuint32_t estr[4] = {1, 1, 1, 1};
-    return fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<double *>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-              CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+    if (fn(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, const_cast<double *>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+           CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return false;
+    Slot &sl = cache[next++ % 8];
+    sl.k = key;
+    sl.m = *map;
+    sl.used = true;
+    return true;
 }
 
 template <int D, int NF, int ORDER, bool NU>
